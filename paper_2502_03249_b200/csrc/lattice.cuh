@@ -1,0 +1,128 @@
+// Lattice geometry, device field layout and memory-access helpers shared by the kernels.
+//
+// Layout (include/qcd.h; "Structure of Arrays ... all even sites are listed first,
+// followed by all odd sites"): idx = x0 + N0 (x1 + N1 (x2 + N2 x3)), cb = idx >> 1, every
+// complex component of a field is one plane of Vh contiguous (re, im) pairs.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace qcd {
+
+struct Lattice {
+    int N0, N1, N2, N3;
+    int h;        // N0 / 2 : checkerboard sites per x0-row
+    int Vh;       // sites per parity
+    int s1;       // cb stride of x1 (= h)
+    int s2;       // cb stride of x2 (= h N1)
+    int s3;       // cb stride of x3 (= h N1 N2)
+};
+
+template <typename T> struct Cplx;
+template <> struct Cplx<double> { typedef double2 type; };
+template <> struct Cplx<float>  { typedef float2 type; };
+
+// L2 eviction policies (createpolicy, PTX ISA): links are read exactly once per half-Dslash
+// (evict_first), neighbour spinors are read by 8 output sites (evict_last).
+__device__ __forceinline__ uint64_t l2_policy_evict_first()
+{
+    uint64_t p;
+    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
+    return p;
+}
+__device__ __forceinline__ uint64_t l2_policy_evict_last()
+{
+    uint64_t p;
+    asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p));
+    return p;
+}
+
+// streaming load: read-only path, no L1 allocation, L2 policy operand
+__device__ __forceinline__ double2 ld_stream(const double2 *p, uint64_t pol)
+{
+    double2 r;
+    asm volatile("ld.global.nc.L1::no_allocate.L2::cache_hint.v2.f64 {%0,%1}, [%2], %3;"
+                 : "=d"(r.x), "=d"(r.y) : "l"(p), "l"(pol));
+    return r;
+}
+__device__ __forceinline__ float2 ld_stream(const float2 *p, uint64_t pol)
+{
+    float2 r;
+    asm volatile("ld.global.nc.L1::no_allocate.L2::cache_hint.v2.f32 {%0,%1}, [%2], %3;"
+                 : "=f"(r.x), "=f"(r.y) : "l"(p), "l"(pol));
+    return r;
+}
+__device__ __forceinline__ float4 ld_stream(const float4 *p, uint64_t pol)
+{
+    float4 r;
+    asm volatile("ld.global.nc.L1::no_allocate.L2::cache_hint.v4.f32 {%0,%1,%2,%3}, [%4], %5;"
+                 : "=f"(r.x), "=f"(r.y), "=f"(r.z), "=f"(r.w) : "l"(p), "l"(pol));
+    return r;
+}
+// reused load: read-only path, L1 allocation allowed, L2 policy operand
+__device__ __forceinline__ double2 ld_keep(const double2 *p, uint64_t pol)
+{
+    double2 r;
+    asm volatile("ld.global.nc.L2::cache_hint.v2.f64 {%0,%1}, [%2], %3;"
+                 : "=d"(r.x), "=d"(r.y) : "l"(p), "l"(pol));
+    return r;
+}
+__device__ __forceinline__ float2 ld_keep(const float2 *p, uint64_t pol)
+{
+    float2 r;
+    asm volatile("ld.global.nc.L2::cache_hint.v2.f32 {%0,%1}, [%2], %3;"
+                 : "=f"(r.x), "=f"(r.y) : "l"(p), "l"(pol));
+    return r;
+}
+__device__ __forceinline__ float4 ld_keep(const float4 *p, uint64_t pol)
+{
+    float4 r;
+    asm volatile("ld.global.nc.L2::cache_hint.v4.f32 {%0,%1,%2,%3}, [%4], %5;"
+                 : "=f"(r.x), "=f"(r.y), "=f"(r.z), "=f"(r.w) : "l"(p), "l"(pol));
+    return r;
+}
+
+// Site geometry of one checkerboard index: coordinates, the 8
+// neighbour checkerboard indices (all in the OTHER parity), Kogut-Susskind phases and the
+// antiperiodic-time seam signs, all from integer arithmetic on (parity, cb).
+struct SiteGeom {
+    int nf[4], nb[4];   // cb of x+mu, x-mu
+    float sf[4], sb[4]; // eta_mu(x) * seam sign of the forward hop ; MINUS eta_mu(x-mu) * seam sign of the backward hop
+};
+
+__device__ __forceinline__ SiteGeom site_geometry(const Lattice &L, int parity, int cb)
+{
+    SiteGeom g;
+    const unsigned ucb = (unsigned)cb;
+    const int xh = (int)(ucb % (unsigned)L.h);
+    unsigned r = ucb / (unsigned)L.h;
+    const int x1 = (int)(r % (unsigned)L.N1);
+    r /= (unsigned)L.N1;
+    const int x2 = (int)(r % (unsigned)L.N2);
+    const int x3 = (int)(r / (unsigned)L.N2);
+    const int rp = (x1 + x2 + x3 + parity) & 1;      // x0 = 2 xh + rp, so x0 & 1 == rp
+
+    // mu = 0: the neighbour sits in the same x0-row of the other parity
+    g.nf[0] = rp ? ((xh + 1 == L.h) ? cb - (L.h - 1) : cb + 1) : cb;
+    g.nb[0] = rp ? cb : ((xh == 0) ? cb + (L.h - 1) : cb - 1);
+    g.nf[1] = (x1 + 1 == L.N1) ? cb - (L.N1 - 1) * L.s1 : cb + L.s1;
+    g.nb[1] = (x1 == 0) ? cb + (L.N1 - 1) * L.s1 : cb - L.s1;
+    g.nf[2] = (x2 + 1 == L.N2) ? cb - (L.N2 - 1) * L.s2 : cb + L.s2;
+    g.nb[2] = (x2 == 0) ? cb + (L.N2 - 1) * L.s2 : cb - L.s2;
+    g.nf[3] = (x3 + 1 == L.N3) ? cb - (L.N3 - 1) * L.s3 : cb + L.s3;
+    g.nb[3] = (x3 == 0) ? cb + (L.N3 - 1) * L.s3 : cb - L.s3;
+
+    // eta_0 = 1, eta_1 = (-1)^{x0}, eta_2 = (-1)^{x0+x1}, eta_3 = (-1)^{x0+x1+x2};
+    // eta_mu does not depend on x_mu, so eta_mu(x-mu) = eta_mu(x) (extents are even).
+    const float e1 = rp ? -1.f : 1.f;
+    const float e2 = ((rp + x1) & 1) ? -1.f : 1.f;
+    const float e3 = ((rp + x1 + x2) & 1) ? -1.f : 1.f;
+    g.sf[0] = 1.f;  g.sb[0] = -1.f;
+    g.sf[1] = e1;   g.sb[1] = -e1;
+    g.sf[2] = e2;   g.sb[2] = -e2;
+    g.sf[3] = (x3 + 1 == L.N3) ? -e3 : e3;           // forward hop across the time seam
+    g.sb[3] = (x3 == 0) ? e3 : -e3;                  // backward hop across the time seam
+    return g;
+}
+
+} // namespace qcd

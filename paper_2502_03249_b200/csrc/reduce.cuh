@@ -1,0 +1,81 @@
+// Deterministic two-stage reduction (north_star (c): "a deterministic two-stage warp-shuffle
+// reduction for dot products"; "dot product involving global reductions").
+//
+// Stage 1: every block reduces its threads' double partial sums in a fixed order
+//          (warp shuffle tree, then the warp sums through shared memory in warp order) and
+//          writes ONE double to partials[blockIdx.x].
+// Stage 2: the block that takes the last ticket (an integer atomic, the only atomic used)
+//          re-reads all partials from L2 and sums them in an order that depends only on the
+//          grid size, never on which block arrived last.  No floating-point atomics, so
+//          results are bitwise reproducible run to run.
+#pragma once
+#include <cuda_runtime.h>
+
+namespace qcd {
+
+// CG recurrence state, resident on the device (north_star (d)).
+struct CgScalars {
+    double rr;        // <r,r> of the current residual
+    double bb;        // <b,b>
+    double pAp;       // <p, M p>
+    double alpha;     // rr / pAp
+    double beta;      // rr_new / rr
+    double tol2bb;    // tol^2 * bb  (stop when rr <= tol2bb)
+    double dot;       // result slot of qcd_re_dot
+    int k;            // M applications done
+    int maxiter;
+    int flag;         // 0 running, 1 converged, 2 maxiter reached, 3 breakdown
+    unsigned ticket;  // last-block ticket, wraps to 0 by itself (atomicInc)
+};
+
+__device__ __forceinline__ double warp_sum(double v)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+    return v;
+}
+
+// Sum over the block; the result is valid in thread 0.  All threads must call it.
+template <int BLOCK>
+__device__ __forceinline__ double block_sum(double v, double *smem /* BLOCK/32 doubles */)
+{
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    v = warp_sum(v);
+    if (lane == 0) smem[w] = v;
+    __syncthreads();
+    double s = 0.0;
+    if (threadIdx.x == 0) {
+#pragma unroll
+        for (int i = 0; i < BLOCK / 32; ++i) s += smem[i];
+    }
+    return s;
+}
+
+// Stage 1 + ticket.  Returns true (in every thread of exactly one block) when this block is
+// the last to finish; that block must then call final_sum.
+template <int BLOCK>
+__device__ __forceinline__ bool publish_partial(double v, double *partials, unsigned *ticket, double *smem, int *smem_flag)
+{
+    const double s = block_sum<BLOCK>(v, smem);
+    if (threadIdx.x == 0) {
+        partials[blockIdx.x] = s;
+        __threadfence();
+        const unsigned t = atomicInc(ticket, gridDim.x - 1);
+        *smem_flag = (t == gridDim.x - 1);
+    }
+    __syncthreads();
+    return *smem_flag != 0;
+}
+
+// Stage 2: fixed-order sum of partials[0 .. n).  Result valid in thread 0.
+template <int BLOCK>
+__device__ __forceinline__ double final_sum(const double *partials, int n, double *smem)
+{
+    __threadfence();
+    double s = 0.0;
+    for (int i = threadIdx.x; i < n; i += BLOCK) s += __ldcg(partials + i);
+    __syncthreads();                       // smem is reused
+    return block_sum<BLOCK>(s, smem);
+}
+
+} // namespace qcd

@@ -1,0 +1,275 @@
+"""GPU parity: the CUDA path (through the C-ABI) against the CPU oracle, element by element,
+on the same seeded inputs.  Tolerances are BASELINE.json north_star's:
+  Dslash  max relative error <= 1e-13 (fp64), <= 2e-6 (fp32)   [per-site measure, R10]
+  CG      oracle-recomputed fp64 true residual <= tol, iterations within 2% of the oracle's
+          [DESIGN.md R8: |d| <= max(2, ceil(0.02 it))]
+For fp32 the reference is the fp64 oracle applied to the fp32-ROUNDED inputs."""
+import numpy as np
+import pytest
+
+import oracle
+import qcd_inputs
+from util import DSLASH_TOL, dslash_rel_err, iters_close
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def q():
+    import paper_2502_03249_b200 as pkg
+    return pkg
+
+
+def _rounded(a, prec):
+    """what the device holds: the fp64 array itself, or its fp32 rounding (as complex128 for the oracle)."""
+    if prec == 64:
+        return a
+    return a.astype(np.complex64).astype(np.complex128)
+
+
+SMALL_LATTICES = [
+    ((4, 4, 4, 4), "haar", None),            # configs[0]
+    ((4, 6, 2, 8), "haar", None),            # ragged: every extent different, N2 = 2 (x+mu == x-mu)
+    ((8, 4, 6, 10), "near_identity", 0.5),   # Vh = 960: several blocks and a ragged tail
+    ((12, 2, 2, 2), "haar", None),           # h = 6: not a power of two, rows shorter than a warp
+]
+
+
+# ------------------------------------------------------------------------------------------
+# layout
+# ------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("prec", [64, 32])
+@pytest.mark.parametrize("dims", [(4, 4, 4, 4), (8, 4, 6, 10), (16, 16, 16, 16)])
+def test_layout_roundtrip_and_plane_order(q, dims, prec):
+    import torch
+    ctx = q.Context(dims, prec)
+    cd = ctx.cdtype
+    U = qcd_inputs.gauge_field(dims, "haar", seed=3).astype(cd)
+    phi = qcd_inputs.gaussian_spinor(dims, seed=4).astype(cd)
+    par = qcd_inputs.site_parity(dims)
+    V = U.shape[0]
+    Vh = V // 2
+
+    fU = ctx.field(q.QCD_GAUGE).upload(U)
+    assert np.array_equal(fU.download(), U)
+    # device layout: [parity][mu][k][cb] with cb = idx >> 1 (include/qcd.h)
+    real = torch.float64 if prec == 64 else torch.float32
+    dev = fU.buf.view(real).view(2, 4, 9, Vh, 2).cpu().numpy()
+    dev = dev[..., 0] + 1j * dev[..., 1]
+    for p in (0, 1):
+        idx = np.nonzero(par == p)[0]
+        assert np.array_equal(idx >> 1, np.arange(Vh))            # cb enumerates the parity's sites in order
+        expect = U[idx].reshape(Vh, 4, 9).transpose(1, 2, 0)
+        assert np.array_equal(dev[p], expect)
+
+    full = ctx.field(q.QCD_SPINOR_FULL).upload(phi)
+    assert np.array_equal(full.download(), phi)
+    sdev = full.buf.view(real).view(2, 3, Vh, 2).cpu().numpy()
+    sdev = sdev[..., 0] + 1j * sdev[..., 1]
+    for p in (0, 1):                                              # even block precedes odd block
+        assert np.array_equal(sdev[p], phi[par == p].T)
+
+    for kind, p in ((q.QCD_SPINOR_EVEN, 0), (q.QCD_SPINOR_ODD, 1)):
+        f = ctx.field(kind).upload(phi)
+        back = f.download()
+        assert np.array_equal(back[par == p], phi[par == p])
+        assert not back[par != p].any()
+    ctx.close()
+
+
+# ------------------------------------------------------------------------------------------
+# Dslash
+# ------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("prec", [64, 32])
+@pytest.mark.parametrize("dims,links,eps", SMALL_LATTICES + [((16, 16, 16, 16), "near_identity", 0.3)])
+def test_dslash_matches_oracle(q, dims, links, eps, prec):
+    ctx = q.Context(dims, prec)
+    U = qcd_inputs.gauge_field(dims, links, seed=0, eps=eps)
+    phi = qcd_inputs.gaussian_spinor(dims, seed=1)
+    par = qcd_inputs.site_parity(dims)
+    Ur, phir = _rounded(U, prec), _rounded(phi, prec)
+    fU = ctx.field(q.QCD_GAUGE).upload(U)
+    fphi = ctx.field(q.QCD_SPINOR_FULL).upload(phi)
+    fout = ctx.field(q.QCD_SPINOR_FULL)
+    fout.buf.zero_()
+    ctx.qcd_dslash_eo(fU, fout, fphi)          # even half of out = D_eo (odd half of phi)
+    ctx.qcd_dslash_oe(fU, fout, fphi)          # odd half of out = D_oe (even half of phi)
+    got = fout.download()
+    ref = oracle.dslash(dims, Ur, phir, -1)    # the full operator D = [[0, D_eo], [D_oe, 0]]
+    for p in (0, 1):
+        err = dslash_rel_err(got[par == p], ref[par == p])
+        assert err <= DSLASH_TOL[prec], (p, err)
+    # separate half-field objects, every variant of the kernel
+    fe = ctx.field(q.QCD_SPINOR_EVEN).upload(phi)
+    fo = ctx.field(q.QCD_SPINOR_ODD)
+    for variant in range(4):
+        ctx.qcd_set_dslash_variant(variant)
+        fo.buf.zero_()
+        ctx.qcd_dslash_oe(fU, fo, fe)
+        got_o = fo.download()
+        assert dslash_rel_err(got_o[par == 1], ref[par == 1]) <= DSLASH_TOL[prec], variant
+        assert not got_o[par == 0].any()
+    ctx.close()
+
+
+@pytest.mark.parametrize("prec", [64, 32])
+@pytest.mark.parametrize("dims,links,eps", SMALL_LATTICES)
+def test_apply_M_matches_oracle(q, dims, links, eps, prec):
+    ctx = q.Context(dims, prec)
+    m = 0.37
+    U = qcd_inputs.gauge_field(dims, links, seed=0, eps=eps)
+    v = qcd_inputs.gaussian_source(dims, seed=5, parity=0)
+    par = qcd_inputs.site_parity(dims)
+    fU = ctx.field(q.QCD_GAUGE).upload(U)
+    fv = ctx.field(q.QCD_SPINOR_EVEN).upload(v)
+    fo = ctx.field(q.QCD_SPINOR_EVEN)
+    ctx.qcd_apply_M(fU, fo, fv, m)
+    got = fo.download()
+    ref = oracle.apply_M(dims, _rounded(U, prec), _rounded(v, prec), m)
+    assert dslash_rel_err(got[par == 0], ref[par == 0]) <= 2 * DSLASH_TOL[prec]   # two hops
+    ctx.close()
+
+
+@pytest.mark.parametrize("prec", [64, 32])
+def test_re_dot_matches_oracle_and_is_deterministic(q, prec):
+    dims = (8, 4, 6, 10)
+    ctx = q.Context(dims, prec)
+    a = qcd_inputs.gaussian_source(dims, seed=6, parity=0)
+    b = qcd_inputs.gaussian_source(dims, seed=7, parity=0)
+    fa = ctx.field(q.QCD_SPINOR_EVEN).upload(a)
+    fb = ctx.field(q.QCD_SPINOR_EVEN).upload(b)
+    got = ctx.qcd_re_dot(fa, fb)
+    ref = oracle.re_dot_even(dims, _rounded(a, prec), _rounded(b, prec))
+    scale = np.sqrt(oracle.re_dot_even(dims, a, a) * oracle.re_dot_even(dims, b, b))
+    assert abs(got - ref) <= 1e-14 * scale
+    assert all(ctx.qcd_re_dot(fa, fb) == got for _ in range(5))
+    ctx.close()
+
+
+# ------------------------------------------------------------------------------------------
+# CG
+# ------------------------------------------------------------------------------------------
+def _solve(q, dims, prec, U, b, m, tol, maxiter):
+    ctx = q.Context(dims, prec)
+    fU = ctx.field(q.QCD_GAUGE).upload(U)
+    fb = ctx.field(q.QCD_SPINOR_EVEN).upload(b)
+    fx = ctx.field(q.QCD_SPINOR_EVEN)
+    info = ctx.qcd_cg_solve(fU, fb, fx, m, tol, maxiter)
+    x = fx.download()
+    ctx.close()
+    return x, info
+
+
+def test_cg_config0_4x4x4x4_fp64(q):
+    cfg, U, b = qcd_inputs.config_inputs(0)
+    dims, m, tol = cfg["dims"], cfg["m"], cfg["tol64"]
+    x, info = _solve(q, dims, 64, U, b, m, tol, cfg["maxiter"])
+    xo, oinfo = oracle.cg(dims, U, b, m, tol, cfg["maxiter"])
+    assert info["status"] == q.QCD_OK and info["converged"]
+    assert oracle.true_residual(dims, U, b, x, m) <= tol
+    assert iters_close(info["iters"], oinfo["iters"]), (info, oinfo)
+    assert info["rel_resid"] <= tol
+    assert abs(info["bnorm2"] - oinfo["bnorm2"]) <= 1e-13 * oinfo["bnorm2"]
+    # both solve the same HPD system to 1e-10: solutions agree to kappa * tol
+    assert np.linalg.norm(x - xo) <= 1e4 * tol * np.linalg.norm(xo)
+
+
+@pytest.mark.parametrize("prec", [64, 32])
+def test_cg_config1_16x16x16x16(q, prec):
+    cfg, U, b = qcd_inputs.config_inputs(1)
+    dims, m = cfg["dims"], cfg["m"]
+    tol = cfg["tol64"] if prec == 64 else cfg["tol32"]
+    x, info = _solve(q, dims, prec, U, b, m, tol, cfg["maxiter"])
+    cd = np.complex128 if prec == 64 else np.complex64
+    Ur, br = U.astype(cd), b.astype(cd)
+    _, oinfo = oracle.cg(dims, Ur, br, m, tol, cfg["maxiter"])      # fp32: the float-arithmetic oracle variant
+    assert info["converged"]
+    assert iters_close(info["iters"], oinfo["iters"]), (info, oinfo)
+    assert oracle.true_residual(dims, Ur, br, x, m) <= tol          # recomputed by the oracle in fp64
+
+
+@pytest.mark.parametrize("prec", [64, 32])
+@pytest.mark.parametrize("dims,links,eps", SMALL_LATTICES[1:])
+def test_cg_small_lattices(q, dims, links, eps, prec):
+    m = 0.2
+    tol = 1e-9 if prec == 64 else 1e-5
+    U = qcd_inputs.gauge_field(dims, links, seed=0, eps=eps)
+    b = qcd_inputs.gaussian_source(dims, seed=1, parity=0)
+    cd = np.complex128 if prec == 64 else np.complex64
+    x, info = _solve(q, dims, prec, U, b, m, tol, 2000)
+    _, oinfo = oracle.cg(dims, U.astype(cd), b.astype(cd), m, tol, 2000)
+    assert info["converged"]
+    assert iters_close(info["iters"], oinfo["iters"]), (info, oinfo)
+    assert oracle.true_residual(dims, U.astype(cd), b.astype(cd), x, m) <= tol
+
+
+def test_cg_is_bitwise_deterministic_and_piecewise_equals_solve(q):
+    cfg, U, b = qcd_inputs.config_inputs(1, dims=(8, 8, 8, 8))
+    dims, m, tol = cfg["dims"], cfg["m"], 1e-10
+    x1, i1 = _solve(q, dims, 64, U, b, m, tol, 1000)
+    x2, i2 = _solve(q, dims, 64, U, b, m, tol, 1000)
+    assert i1["iters"] == i2["iters"] and i1["rel_resid"] == i2["rel_resid"]
+    assert np.array_equal(x1, x2)
+    # begin / iterate / finish, over-launching far past convergence: x frozen at the exact iteration
+    ctx = q.Context(dims, 64)
+    fU = ctx.field(q.QCD_GAUGE).upload(U)
+    fb = ctx.field(q.QCD_SPINOR_EVEN).upload(b)
+    fx = ctx.field(q.QCD_SPINOR_EVEN)
+    ctx.qcd_cg_begin(fU, fb, fx, m, tol, 1000)
+    ctx.qcd_cg_iterate(7)
+    state, it, rr = ctx.qcd_cg_poll()
+    assert (state, it) == (0, 7) and 0 < rr < 1
+    ctx.qcd_cg_iterate(i1["iters"] + 50)
+    i3 = ctx.qcd_cg_finish()
+    assert i3["iters"] == i1["iters"] and i3["converged"]
+    assert np.array_equal(fx.download(), x1)
+    ctx.close()
+
+
+def test_cg_edge_cases(q):
+    dims = (4, 4, 4, 4)
+    cfg, U, b = qcd_inputs.config_inputs(0)
+    ctx = q.Context(dims, 64)
+    fU = ctx.field(q.QCD_GAUGE).upload(U)
+    fb = ctx.field(q.QCD_SPINOR_EVEN).upload(b)
+    fx = ctx.field(q.QCD_SPINOR_EVEN)
+    fodd = ctx.field(q.QCD_SPINOR_ODD)
+    # b = 0 -> x = 0, 0 iterations, converged
+    fz = ctx.field(q.QCD_SPINOR_EVEN).upload(np.zeros_like(b))
+    fx.buf.fill_(255)
+    info = ctx.qcd_cg_solve(fU, fz, fx, 0.1, 1e-10, 100)
+    assert info["status"] == q.QCD_OK and info["iters"] == 0 and not fx.download().any()
+    # maxiter = 0 -> x = 0, not converged
+    info = ctx.qcd_cg_solve(fU, fb, fx, 0.1, 1e-10, 0)
+    assert info["status"] == q.QCD_ENOTCONVERGED and info["iters"] == 0 and not fx.download().any()
+    # maxiter reached: exactly maxiter M applications, x = that iterate of the oracle's sequence
+    info = ctx.qcd_cg_solve(fU, fb, fx, 0.1, 1e-10, 13)
+    assert info["status"] == q.QCD_ENOTCONVERGED and info["iters"] == 13 and not info["converged"]
+    xo, oinfo = oracle.cg(dims, U, b, 0.1, 1e-10, 13)
+    assert oinfo["iters"] == 13
+    assert np.linalg.norm(fx.download() - xo) <= 1e-10 * np.linalg.norm(xo)
+    assert abs(info["rel_resid"] - oinfo["rel_resid"]) <= 1e-9 * oinfo["rel_resid"]
+    # large mass: x ~ b / m^2 in O(1) iterations
+    info = ctx.qcd_cg_solve(fU, fb, fx, 100.0, 1e-10, 100)
+    assert info["converged"] and info["iters"] <= 6
+    assert np.linalg.norm(fx.download() - b / 1e4) <= 1e-2 * np.linalg.norm(b / 1e4)
+    # argument errors
+    for bad in (dict(m=-1.0), dict(tol=0.0), dict(maxiter=-1)):
+        kw = dict(m=0.1, tol=1e-8, maxiter=10)
+        kw.update(bad)
+        with pytest.raises(q.QcdError) as e:
+            ctx.qcd_cg_solve(fU, fb, fx, **kw)
+        assert e.value.status == q.QCD_EINVAL
+    with pytest.raises(q.QcdError):
+        ctx.qcd_cg_solve(fU, fb, fb, 0.1, 1e-8, 10)        # x aliases b
+    with pytest.raises(q.QcdError):
+        ctx.qcd_cg_solve(fU, fodd, fx, 0.1, 1e-8, 10)      # wrong parity
+    with pytest.raises(q.QcdError):
+        ctx.qcd_dslash_eo(fU, fodd, fb)                    # swapped parities
+    with pytest.raises(q.QcdError):
+        ctx.qcd_dslash_oe(fb, fodd, fb)                    # U is not a gauge field
+    with pytest.raises(q.QcdError):
+        ctx.qcd_apply_M(fU, fb, fb, 0.1)                   # aliasing
+    ctx.close()
+    with pytest.raises(q.QcdError):
+        q.Context((4, 4, 5, 4), 64)
