@@ -1,0 +1,412 @@
+#!/usr/bin/env python
+"""bench.py -- staggered Dslash + CG hot path on B200 (one JSON line on stdout; rank 0 only).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--lattice 64,64,64,64] [--quick]
+
+Workload (config.workload): BASELINE.json configs[4] -- 64^4 lattice, Haar-random SU(3) links
+(seed 0), Gaussian even-site source (seed 1), m = 0.01, fp64 -- the configuration the metric is
+quoted on.  Inputs (9.7 GB of links) are far larger than the 126 MB L2, so no L2 flush is needed
+between timed iterations.
+
+A STEP is one Conjugate-Gradient iteration on M = m^2 - D_eo D_oe = one pass over every row of
+SURVEY.md Sec. 8(a): D_oe, D_eo + M epilogue + <p,Mp>, alpha, fused x/r update + |r|^2, beta and
+the stop test, the p update -- all in our CUDA kernels, scalars resident on the device.
+
+  value : effective GB/s = nominal bytes of one iteration (3648 B per even site in fp64:
+          two half-Dslash at 1584 B/site (BASELINE.json north_star) + 480 B of vector traffic)
+          x sites x K / device time of K iterations.  Inputs resident in HBM.
+  e2e   : the same K iterations through the C-ABI with HOST buffers: qcd_field_upload of the
+          source from pinned memory, K x (qcd_cg_iterate(1) + qcd_cg_poll, a 72-byte D2H read
+          of the residual after every step), qcd_field_download of the iterate to pinned memory.
+  roofline : the Dslash kernel (D_oe launches inside the timed region, CUDA events on the
+          launching stream), algorithmic = COMPULSORY DRAM bytes 1248 B/site (each link once,
+          each spinor once, one store), against MEASURED_PEAKS.json hbm_gbs.
+  cpu_baseline / --impl reference : the CPU oracle as it stands on the host cores.
+
+N > 1: replicas only: every rank runs the same workload on its own
+GPU, no data-path collective; value = sum of units / max-over-ranks device time.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+# ---- byte / flop model -------------------
+FLOP_PER_SITE = 570
+REALS_DSLASH_NOMINAL = 198               # 8 links x 18 + 8 vectors x 6 + 1 vector written (north_star: 1584 B fp64)
+REALS_DSLASH_COMPULSORY = 156            # 8 links x 18 + 1 vector read + 1 written          (1248 B fp64)
+REALS_ITER_NOMINAL = 2 * 198 + 6 + 36 + 18      # + epilogue read of p, x/r update (6 vectors), p update (3 vectors) = 456
+REALS_ITER_COMPULSORY = 2 * 156 + 6 + 36 + 18   # = 372 (2976 B fp64)
+THEORETICAL_HBM_GBS = 8184.0             # 3996 MHz x 2 (DDR) x 8192 bit / 8 -- nvidia-smi max memory clock; context only
+
+METRIC = "staggered CG-iteration effective GB/s (two half-Dslash at 1584 B/site + CG vector kernels), 64^4 fp64"
+UNIT = "GB/s"
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours", choices=("ours", "reference"))
+    ap.add_argument("--lattice", default=None, help="override dims, e.g. 16,16,16,16 (testing only)")
+    ap.add_argument("--quick", action="store_true", help="skip the extra reports (full solves, fp32, cpu_baseline)")
+    return ap.parse_args()
+
+
+def load_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            d = json.load(f)
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, torch copy)"
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def load_traffic(prec: int):
+    """ncu-measured DRAM bytes per Dslash launch, recorded in profiles/ (text, committed); None if absent."""
+    p = os.path.join(ROOT, "profiles", "dslash_traffic.json")
+    if not os.path.exists(p):
+        return None
+    with open(p) as f:
+        d = json.load(f)
+    return d.get(f"fp{prec}_64x64x64x64_bytes_per_launch")
+
+
+# ---- clocks ---------------------------------------------------------------------------------
+class ClockSampler:
+    """Samples SM clock and throttle reasons through NVML while the timed region runs."""
+
+    def __init__(self, index: int):
+        self.samples, self.reasons, self.max_mhz = [], set(), None
+        self._stop = threading.Event()
+        self._thr = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+        except Exception as e:  # pragma: no cover
+            self.nv, self.err = None, repr(e)
+
+    def _run(self):
+        nv = self.nv
+        names = {
+            "hw_slowdown": getattr(nv, "nvmlClocksEventReasonHwSlowdown", 0x8),
+            "hw_thermal_slowdown": getattr(nv, "nvmlClocksEventReasonHwThermalSlowdown", 0x40),
+            "sw_thermal_slowdown": getattr(nv, "nvmlClocksEventReasonSwThermalSlowdown", 0x20),
+            "sw_power_cap": getattr(nv, "nvmlClocksEventReasonSwPowerCap", 0x4),
+            "hw_power_brake": getattr(nv, "nvmlClocksEventReasonHwPowerBrakeSlowdown", 0x80),
+        }
+        while not self._stop.is_set():
+            try:
+                self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                try:
+                    r = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)
+                except Exception:
+                    r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                for k, bit in names.items():
+                    if r & bit:
+                        self.reasons.add(k)
+            except Exception:
+                pass
+            time.sleep(0.01)
+
+    def __enter__(self):
+        if self.nv:
+            self._thr = threading.Thread(target=self._run, daemon=True)
+            self._thr.start()
+        return self
+
+    def __exit__(self, *a):
+        self._stop.set()
+        if self._thr:
+            self._thr.join()
+
+    def summary(self):
+        if not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons), "samples": 0}
+        return {"sm_mhz": float(np.median(self.samples)), "sm_max_mhz": self.max_mhz,
+                "reasons": sorted(self.reasons), "samples": len(self.samples)}
+
+
+# ---- multi-rank plumbing ---------------------------------------------------------------------
+def dist_env():
+    return int(os.environ.get("RANK", 0)), int(os.environ.get("LOCAL_RANK", 0)), int(os.environ.get("WORLD_SIZE", 1))
+
+
+def aggregate_over_ranks(local_ms: float, local_units: float, backend_device=None):
+    """(max-over-ranks time, sum-over-ranks units).  No data-path collective exists; this is the
+    only communication in the bench.  Works with gloo (CPU tensors) and nccl (CUDA tensors)."""
+    import torch
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()):
+        return local_ms, local_units
+    dev = backend_device if backend_device is not None else "cpu"
+    t = torch.tensor([local_ms], dtype=torch.float64, device=dev)
+    u = torch.tensor([local_units], dtype=torch.float64, device=dev)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    dist.all_reduce(u, op=dist.ReduceOp.SUM)
+    return float(t.item()), float(u.item())
+
+
+# ---- our arm ---------------------------------------------------------------------------------
+def make_inputs(dims, cfg_index=4):
+    import qcd_inputs
+    cfg = dict(qcd_inputs.CONFIGS[cfg_index])
+    cfg["dims"] = tuple(dims)
+    U = qcd_inputs.gauge_field(cfg["dims"], cfg["links"], seed=0, eps=cfg["eps"])
+    b = qcd_inputs.gaussian_source(cfg["dims"], seed=1, parity=0)
+    return cfg, U, b
+
+
+def time_dslash(q, torch, ctx, fU, fin, fout, n=20):
+    for _ in range(3):
+        ctx.qcd_dslash_oe(fU, fout, fin)
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(n):
+        ctx.qcd_dslash_oe(fU, fout, fin)
+    e1.record()
+    torch.cuda.synchronize()
+    return e0.elapsed_time(e1) / n
+
+
+def dslash_report(ms, Vh, rsize, peak):
+    comp = REALS_DSLASH_COMPULSORY * rsize * Vh / ms / 1e6
+    return {"ms": round(ms, 5), "gflops": round(FLOP_PER_SITE * Vh / ms / 1e6, 1),
+            "effective_gbs_nominal": round(REALS_DSLASH_NOMINAL * rsize * Vh / ms / 1e6, 1),
+            "gbs_compulsory": round(comp, 1),
+            "frac_of_measured_copy_peak": round(comp / peak, 4),
+            "frac_of_theoretical_8184": round(comp / THEORETICAL_HBM_GBS, 4)}
+
+
+def run_ours(args):
+    import torch
+    import paper_2502_03249_b200 as q
+
+    rank, local_rank, world = dist_env()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    dev = f"cuda:{local_rank}"
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device(dev))
+
+    dims = tuple(int(v) for v in args.lattice.split(",")) if args.lattice else (64, 64, 64, 64)
+    K, W = args.steps, args.warmup
+    peak, peak_src = load_peaks()
+    t_setup = time.time()
+    cfg, U, b = make_inputs(dims)
+    V = int(np.prod(dims))
+    Vh = V // 2
+    m, tol64 = cfg["m"], cfg["tol64"]
+
+    ctx = q.Context(dims, 64, device=dev)
+    fU = ctx.field(q.QCD_GAUGE).upload(U)
+    fb = ctx.field(q.QCD_SPINOR_EVEN).upload(b)
+    fx = ctx.field(q.QCD_SPINOR_EVEN)
+    fo = ctx.field(q.QCD_SPINOR_ODD)
+    t_setup = time.time() - t_setup
+
+    def barrier():
+        if world > 1:
+            import torch.distributed as dist
+            dist.barrier()
+
+    # ---------------- timed region: K CG iterations, inputs resident --------------------------
+    ctx.qcd_cg_begin(fU, fb, fx, m, 1e-300, 1 << 30)      # tol far below reach: every step does full work
+    ctx.qcd_cg_iterate(W)
+    barrier()
+    torch.cuda.synchronize()
+    ctx.qcd_profile_enable(True)
+    launches0 = ctx.qcd_launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    with ClockSampler(local_rank) as clocks:
+        e0.record()
+        ctx.qcd_cg_iterate(K)
+        e1.record()
+        torch.cuda.synchronize()
+    barrier()
+    ms_total = e0.elapsed_time(e1)
+    launches = ctx.qcd_launch_count() - launches0
+    prof = {k: ctx.qcd_profile_read(k) for k in range(4)}
+    ctx.qcd_profile_enable(False)
+    state, it_done, _ = ctx.qcd_cg_poll()
+    ctx.qcd_cg_finish()
+    assert state == 0 and it_done == W + K, (state, it_done)
+
+    bytes_iter = REALS_ITER_NOMINAL * 8 * Vh
+    ms_max, units = aggregate_over_ranks(ms_total, float(K) * bytes_iter, dev if world > 1 else None)
+    value = units / ms_max / 1e6
+
+    # ---------------- e2e: host buffers through the C-ABI --------------------------------------
+    hb = torch.from_numpy(b).pin_memory()
+    hx = torch.empty_like(hb).pin_memory()
+    torch.cuda.synchronize()
+    barrier()
+    t0 = time.perf_counter()
+    e0.record()
+    ctx._check(ctx.lib.qcd_field_upload(fb.handle, hb.data_ptr()), "qcd_field_upload")
+    ctx.qcd_cg_begin(fU, fb, fx, m, 1e-300, 1 << 30)
+    rr_last = None
+    for _ in range(K):
+        ctx.qcd_cg_iterate(1)
+        _, _, rr_last = ctx.qcd_cg_poll()                  # D2H read of the step's result (residual)
+    ctx.qcd_cg_finish()
+    ctx._check(ctx.lib.qcd_field_download(fx.handle, hx.data_ptr()), "qcd_field_download")
+    e1.record()
+    torch.cuda.synchronize()
+    e2e_wall_ms = (time.perf_counter() - t0) * 1e3
+    e2e_ms = e0.elapsed_time(e1)
+    e2e_ms_max, e2e_units = aggregate_over_ranks(max(e2e_ms, e2e_wall_ms), float(K) * bytes_iter, dev if world > 1 else None)
+    spinor_host_bytes = hb.numel() * hb.element_size()
+    e2e = {"value": round(e2e_units / e2e_ms_max / 1e6, 2), "unit": UNIT,
+           "h2d_bytes_per_step": int(spinor_host_bytes / K), "d2h_bytes_per_step": int(spinor_host_bytes / K + 72),
+           "ms_total": round(e2e_ms_max, 3),
+           "what": "qcd_field_upload(b, pinned host) + K x [qcd_cg_iterate(1) + qcd_cg_poll (D2H of the residual)] + "
+                   "qcd_field_download(x, pinned host); host copies amortised over the K steps of the solve"}
+    del hb, hx
+
+    # ---------------- roofline of the dominant kernel ------------------------------------------
+    n_ds, ms_ds = prof[q.QCD_K_DSLASH]
+    ds_ms = ms_ds / max(n_ds, 1)
+    achieved = REALS_DSLASH_COMPULSORY * 8 * Vh / ds_ms / 1e6
+    roofline = {"bound": "hbm", "kernel": "dslash_kernel<double,MODE0> (D_oe inside the CG iteration)",
+                "achieved": round(achieved, 1), "peak": peak, "unit": "GB/s", "frac": round(achieved / peak, 4),
+                "peak_source": peak_src, "traffic": load_traffic(64),
+                "algorithmic_bytes_per_launch": REALS_DSLASH_COMPULSORY * 8 * Vh,
+                "avg_launch_ms": round(ds_ms, 5), "launches_timed": n_ds,
+                "frac_of_theoretical_8184": round(achieved / THEORETICAL_HBM_GBS, 4)}
+    kernel_ms = {name: round(prof[k][1] / max(prof[k][0], 1), 5) for name, k in
+                 (("dslash_oe", q.QCD_K_DSLASH), ("dslash_eo_epilogue_dot", q.QCD_K_DSLASH_EPI),
+                  ("update_xr_norm", q.QCD_K_UPDATE_XR), ("update_p", q.QCD_K_UPDATE_P))}
+
+    out = {
+        "metric": METRIC, "value": round(value, 2), "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+        "ms_per_step": round(ms_max / K, 5), "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic (seeded Haar SU(3) links, Gaussian source; BASELINE.json configs[4])",
+        "config": {"workload": f"{'x'.join(map(str, dims))} staggered CG iteration, Haar links, m={m}, fp64, full 18-real links",
+                   "lattice": list(dims), "sites": V, "l2": "inputs (9.7 GB links) >> 126 MB L2, no flush needed",
+                   "parallelism": "replicas only (no data-path collective)" if world > 1 else "single GPU",
+                   "bytes_per_even_site_per_step": REALS_ITER_NOMINAL * 8},
+        "clocks": clocks.summary(), "e2e": e2e, "gpu_launches": int(launches),
+        "roofline": roofline, "kernel_ms": kernel_ms, "setup_seconds": round(t_setup, 1),
+    }
+
+    if rank == 0 and not args.quick:
+        extras(args, q, torch, ctx, out, cfg, dims, U, b, fU, fb, fx, fo, peak)
+    if rank == 0:
+        print(json.dumps(out), flush=True)
+    ctx.close()
+    if world > 1:
+        import torch.distributed as dist
+        dist.destroy_process_group()
+
+
+def extras(args, q, torch, ctx, out, cfg, dims, U, b, fU, fb, fx, fo, peak):
+    """Reports beside the headline (rank 0, N = 1 semantics): Dslash alone, full solves, fp32, oracle."""
+    import oracle
+    V = int(np.prod(dims))
+    Vh = V // 2
+    m = cfg["m"]
+    # Dslash alone, fp64
+    out["dslash_fp64"] = dslash_report(time_dslash(q, torch, ctx, fU, fb, fo), Vh, 8, peak)
+    # full fp64 solve: CG s/solve (BASELINE.json metric)
+    info = ctx.qcd_cg_solve(fU, fb, fx, m, cfg["tol64"], cfg["maxiter"])
+    x64 = fx.download()
+    t0 = time.time()
+    true64 = oracle.true_residual(dims, U, b, x64, m)
+    t_true = time.time() - t0
+    out["cg_fp64"] = {"tol": cfg["tol64"], "iters": info["iters"], "converged": info["converged"],
+                      "s_per_solve": round(info["seconds"], 4),
+                      "ms_per_iter": round(1e3 * info["seconds"] / max(info["iters"], 1), 5),
+                      "rel_resid_recurrence": info["rel_resid"], "true_resid_oracle_fp64": true64}
+    # CPU baseline: the oracle as it stands, a bounded sample of the same workload
+    nit = 3
+    t0 = time.time()
+    _, oinfo = oracle.cg(dims, U, b, m, 1e-300, nit)
+    t_or = time.time() - t0
+    out["cpu_baseline"] = {"value": round(REALS_ITER_NOMINAL * 8 * Vh * oinfo["iters"] / t_or / 1e9, 3), "unit": UNIT,
+                           "cores": oracle.num_threads(), "kind": "oracle",
+                           "sample": f"{nit} CG iterations (maxiter={nit}) of the same {'x'.join(map(str, dims))} fp64 solve, "
+                                     f"including the oracle's own set-up; {t_or:.1f} s",
+                           "oracle_apply_M_seconds": round(t_true, 2)}
+    del x64
+    # fp32: free the fp64 device fields first
+    fU.free(); fb.free(); fx.free(); fo.free()
+    ctx.close()
+    torch.cuda.empty_cache()
+    c32 = q.Context(dims, 32, device=ctx.device)
+    U32, b32 = U.astype(np.complex64), b.astype(np.complex64)
+    gU = c32.field(q.QCD_GAUGE).upload(U32)
+    gb = c32.field(q.QCD_SPINOR_EVEN).upload(b32)
+    gx = c32.field(q.QCD_SPINOR_EVEN)
+    go = c32.field(q.QCD_SPINOR_ODD)
+    out["dslash_fp32"] = dslash_report(time_dslash(q, torch, c32, gU, gb, go), Vh, 4, peak)
+    if cfg["tol32"]:
+        info = c32.qcd_cg_solve(gU, gb, gx, m, cfg["tol32"], cfg["maxiter"])
+        x32 = gx.download()
+        out["cg_fp32"] = {"tol": cfg["tol32"], "iters": info["iters"], "converged": info["converged"],
+                          "s_per_solve": round(info["seconds"], 4),
+                          "ms_per_iter": round(1e3 * info["seconds"] / max(info["iters"], 1), 5),
+                          "rel_resid_recurrence": info["rel_resid"],
+                          "true_resid_oracle_fp64": oracle.true_residual(dims, U32, b32, x32, m),
+                          "note": "plain fp32 CG on Haar links stalls in TRUE residual near 1e-4 (DESIGN.md R11)"}
+    c32.close()
+    out["paper_context"] = {"A100_OpenCL_dslash_fp64_TFLOPs_32^4_12real_links_gaugefixed": 1.245,
+                            "A100_OpenCL_cg_update_GBs_48^4_fp64": 1351, "source": "PAPER.md:59,87 (other hardware; context only)"}
+
+
+# ---- reference arm: the CPU oracle -------------------------------------------------------------
+def run_reference(args):
+    rank, _, world = dist_env()
+    if rank != 0:
+        return
+    import oracle
+    K, W = args.steps, args.warmup
+    dims = tuple(int(v) for v in args.lattice.split(",")) if args.lattice else (32, 32, 32, 32)
+    cfg, U, b = make_inputs(dims)
+    Vh = int(np.prod(dims)) // 2
+    if W > 0:
+        oracle.cg(dims, U, b, cfg["m"], 1e-300, W)
+    t0 = time.perf_counter()
+    _, info = oracle.cg(dims, U, b, cfg["m"], 1e-300, K)
+    dt = time.perf_counter() - t0
+    value = REALS_ITER_NOMINAL * 8 * Vh * info["iters"] / dt / 1e9
+    sample = (f"{K} CG iterations of the CPU oracle on a {'x'.join(map(str, dims))} lattice of the same recipe "
+              f"(Haar links, m={cfg['m']}, fp64): a 1/{(64 ** 4) // int(np.prod(dims))} sample of the 64^4 sites; GB/s is per-site intensive")
+    out = {"impl": "reference", "metric": METRIC, "value": round(value, 4), "unit": UNIT, "n_gpus": world, "steps": K,
+           "warmup": W, "ms_per_step": round(1e3 * dt / max(info["iters"], 1), 3), "higher_is_better": True,
+           "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic (seeded)",
+           "config": {"workload": "64x64x64x64 staggered CG iteration, Haar links, m=0.01, fp64, full 18-real links",
+                      "sample": sample},
+           "cpu_baseline": {"value": round(value, 4), "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle", "sample": sample},
+           "e2e": {"value": round(value, 4), "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+           "gpu_launches": 0}
+    print(json.dumps(out), flush=True)
+
+
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

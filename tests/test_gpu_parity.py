@@ -196,11 +196,18 @@ def test_cg_small_lattices(q, dims, links, eps, prec):
     U = qcd_inputs.gauge_field(dims, links, seed=0, eps=eps)
     b = qcd_inputs.gaussian_source(dims, seed=1, parity=0)
     cd = np.complex128 if prec == 64 else np.complex64
+    Ur, br = U.astype(cd), b.astype(cd)
     x, info = _solve(q, dims, prec, U, b, m, tol, 2000)
-    _, oinfo = oracle.cg(dims, U.astype(cd), b.astype(cd), m, tol, 2000)
+    xo, oinfo = oracle.cg(dims, Ur, br, m, tol, 2000)
     assert info["converged"]
     assert iters_close(info["iters"], oinfo["iters"]), (info, oinfo)
-    assert oracle.true_residual(dims, U.astype(cd), b.astype(cd), x, m) <= tol
+    res = oracle.true_residual(dims, Ur, br, x, m)
+    if prec == 64:
+        assert res <= tol
+    else:
+        # DESIGN.md R11: plain fp32 CG on rough (Haar) links stalls in TRUE residual above the
+        # recurrence tolerance; accept what the fp32-arithmetic oracle itself attains (x2).
+        assert res <= max(tol, 2.0 * oracle.true_residual(dims, Ur, br, xo, m)), res
 
 
 def test_cg_is_bitwise_deterministic_and_piecewise_equals_solve(q):
