@@ -75,12 +75,13 @@ def load_peaks():
 
 def load_traffic(prec: int):
     """ncu-measured DRAM bytes per Dslash launch, recorded in profiles/ (text, committed); None if absent."""
-    p = os.path.join(ROOT, "profiles", "dslash_traffic.json")
+    p = os.path.join(ROOT, "profiles", "dslash_traffic.csv")
     if not os.path.exists(p):
         return None
     with open(p) as f:
-        d = json.load(f)
-    return d.get(f"fp{prec}_64x64x64x64_bytes_per_launch")
+        rows = dict(line.strip().split(",", 1) for line in f if "," in line)
+    v = rows.get(f"fp{prec}_64x64x64x64_bytes_per_launch")
+    return int(v) if v is not None else None
 
 
 # ---- clocks ---------------------------------------------------------------------------------
@@ -287,7 +288,7 @@ def run_ours(args):
     achieved = REALS_DSLASH_COMPULSORY * 8 * Vh / ds_ms / 1e6
     roofline = {"bound": "hbm", "kernel": "dslash_kernel<double,MODE0> (D_oe inside the CG iteration)",
                 "achieved": round(achieved, 1), "peak": peak, "unit": "GB/s", "frac": round(achieved / peak, 4),
-                "peak_source": peak_src, "traffic": load_traffic(64),
+                "peak_source": peak_src, "traffic": load_traffic(64) if dims == (64, 64, 64, 64) else None,
                 "algorithmic_bytes_per_launch": REALS_DSLASH_COMPULSORY * 8 * Vh,
                 "avg_launch_ms": round(ds_ms, 5), "launches_timed": n_ds,
                 "frac_of_theoretical_8184": round(achieved / THEORETICAL_HBM_GBS, 4)}

@@ -1,0 +1,164 @@
+"""GPU parity at BASELINE.json's full sizes (configs 2, 3, 4), in the launch configuration
+bench.py times (default Dslash variant, qcd_cg_solve as bench.py's extras call it).
+
+Dslash: the whole output field against the oracle where the oracle finishes in seconds, plus
+sampled sites through oracle.dslash_site (the literal single-site Eq. (1)), chosen to include
+every lattice face (wrap in each direction, the antiperiodic time seam) and random interior
+sites.  CG: the fp64 oracle recomputes ||b - M x_gpu|| / ||b|| (one M application); the
+iteration count is compared with the oracle's stored count (tests/golden/cg_config*_fp*.json,
+written by tests/golden/make_cg_golden.py from oracle/ only; the fingerprint proves the
+inputs regenerated here are the ones the oracle solved)."""
+import importlib.util
+import json
+import os
+
+import numpy as np
+import pytest
+
+import oracle
+import qcd_inputs
+from util import DSLASH_TOL, dslash_rel_err, iters_close
+
+pytestmark = pytest.mark.gpu
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+_spec = importlib.util.spec_from_file_location("make_cg_golden", os.path.join(HERE, "golden", "make_cg_golden.py"))
+golden_mod = importlib.util.module_from_spec(_spec)
+_spec.loader.exec_module(golden_mod)
+
+
+@pytest.fixture(scope="module")
+def q():
+    import paper_2502_03249_b200 as pkg
+    return pkg
+
+
+_cache = {}
+
+
+def inputs(i):
+    """One config's inputs at a time (64^4 links are 9.7 GB on the host)."""
+    if _cache.get("i") != i:
+        _cache.clear()
+        cfg, U, b = qcd_inputs.config_inputs(i)
+        _cache.update(i=i, cfg=cfg, U=U, b=b, fp=golden_mod.fingerprint(U, b))
+    return _cache["cfg"], _cache["U"], _cache["b"]
+
+
+def golden(i, prec):
+    p = golden_mod.golden_path(i, prec)
+    if not os.path.exists(p):
+        return None
+    with open(p) as f:
+        g = json.load(f)
+    assert g["input_fingerprint"] == _cache["fp"], "inputs regenerated here differ from the ones the oracle solved"
+    return g
+
+
+def sample_sites(dims, parity, n_random, seed):
+    """Sites of one parity: all 2^4 combinations of {first, last} coordinate per direction that have
+    the parity (faces, edges, corners: every wrap and the time seam), plus random ones."""
+    rng = np.random.default_rng(seed)
+    sites = []
+    for c in np.ndindex(2, 2, 2, 2):
+        x = [0 if c[d] == 0 else dims[d] - 1 for d in range(4)]
+        for bump in range(2):                       # the corner and its x0-neighbour cover both parities
+            y = list(x)
+            y[0] = (y[0] + bump) % dims[0]
+            if sum(y) % 2 == parity:
+                sites.append(tuple(y))
+    while len(sites) < n_random + 16:
+        x = [int(rng.integers(0, d)) for d in dims]
+        if sum(x) % 2 == parity:
+            sites.append(tuple(x))
+    return sites
+
+
+def lex(dims, x):
+    return x[0] + dims[0] * (x[1] + dims[1] * (x[2] + dims[2] * x[3]))
+
+
+def rounded(a, prec):
+    return a if prec == 64 else a.astype(np.complex64).astype(np.complex128)
+
+
+# ------------------------------------------------------------------------------------------
+# Dslash at full size
+# ------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("prec", [64, 32])
+@pytest.mark.parametrize("config", [2, 3, 4])
+def test_dslash_full_size(q, config, prec):
+    cfg, U, b = inputs(config)
+    dims = cfg["dims"]
+    if prec == 32 and cfg["tol32"] is None:
+        pytest.skip("BASELINE.json names fp64 only for this config")
+    V = int(np.prod(dims))
+    ctx = q.Context(dims, prec)
+    fU = ctx.field(q.QCD_GAUGE).upload(U)
+    fe = ctx.field(q.QCD_SPINOR_EVEN).upload(b)
+    fo = ctx.field(q.QCD_SPINOR_ODD)
+    fe2 = ctx.field(q.QCD_SPINOR_EVEN)
+    ctx.qcd_dslash_oe(fU, fo, fe)              # t = D_oe b
+    ctx.qcd_dslash_eo(fU, fe2, fo)             # D_eo t
+    got_o = fo.download()
+    got_e = fe2.download()
+    Ur, br = rounded(U, prec), rounded(b, prec)
+    tol = DSLASH_TOL[prec]
+    R_o = np.sqrt(np.mean(np.linalg.norm(got_o[1::2], axis=1) ** 2))      # rms site norm scale (R10)
+    # sampled sites, literal Eq. (1) one site at a time
+    worst = 0.0
+    for x in sample_sites(dims, 1, 300, seed=config):
+        ref = oracle.dslash_site(dims, Ur, br, x)
+        d = np.linalg.norm(got_o[lex(dims, x)] - ref) / max(np.linalg.norm(ref), 0.1 * R_o)
+        worst = max(worst, d)
+    assert worst <= tol, worst
+    # second hop: the oracle is applied to what the device holds for t (already in device precision)
+    t_in = got_o.astype(np.complex128)
+    R_e = np.sqrt(np.mean(np.linalg.norm(got_e[::2], axis=1) ** 2))
+    worst = 0.0
+    for x in sample_sites(dims, 0, 300, seed=100 + config):
+        ref = oracle.dslash_site(dims, Ur, t_in, x)
+        d = np.linalg.norm(got_e[lex(dims, x)] - ref) / max(np.linalg.norm(ref), 0.1 * R_e)
+        worst = max(worst, d)
+    assert worst <= tol, worst
+    # whole field, element by element
+    par = qcd_inputs.site_parity(dims)
+    ref_o = oracle.dslash(dims, Ur, br, 1)
+    assert dslash_rel_err(got_o[par == 1], ref_o[par == 1]) <= tol
+    assert not got_o[par == 0].any()
+    del ref_o
+    ref_e = oracle.dslash(dims, Ur, t_in, 0)
+    assert dslash_rel_err(got_e[par == 0], ref_e[par == 0]) <= tol
+    assert V == par.size
+    ctx.close()
+
+
+# ------------------------------------------------------------------------------------------
+# CG at full size
+# ------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("config,prec", [(2, 64), (2, 32), (3, 64), (4, 64), (4, 32)])
+def test_cg_full_size(q, config, prec):
+    cfg, U, b = inputs(config)
+    dims, m = cfg["dims"], cfg["m"]
+    tol = cfg["tol64"] if prec == 64 else cfg["tol32"]
+    g = golden(config, prec)
+    ctx = q.Context(dims, prec)
+    fU = ctx.field(q.QCD_GAUGE).upload(U)
+    fb = ctx.field(q.QCD_SPINOR_EVEN).upload(b)
+    fx = ctx.field(q.QCD_SPINOR_EVEN)
+    info = ctx.qcd_cg_solve(fU, fb, fx, m, tol, cfg["maxiter"])
+    x = fx.download()
+    ctx.close()
+    assert info["status"] == q.QCD_OK and info["converged"], info
+    assert info["rel_resid"] <= tol
+    true = oracle.true_residual(dims, rounded(U, prec), rounded(b, prec), x, m)
+    if prec == 64:
+        assert true <= tol, true                                  # north_star: recomputed by the oracle in fp64
+    elif g is not None:
+        assert true <= 2.0 * g["true_resid"], (true, g["true_resid"])   # DESIGN.md R11 (Haar links, plain fp32)
+    if g is None:
+        pytest.skip(f"no stored oracle solve for config {config} fp{prec} (tests/golden/make_cg_golden.py); "
+                    f"residual check passed: true {true:.3e}, iters {info['iters']}")
+    assert g["tol"] == tol and g["m"] == m and g["status"] == 0
+    assert iters_close(info["iters"], g["iters"]), (info["iters"], g["iters"])
+    assert abs(info["bnorm2"] - g["bnorm2"]) <= 1e-6 * g["bnorm2"]
