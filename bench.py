@@ -185,6 +185,101 @@ def time_dslash(q, torch, ctx, fU, fin, fout, n=20):
     return e0.elapsed_time(e1) / n
 
 
+def variant_reals(nrow, tg, n, N3):
+    """(compulsory, nominal) reals per output site of one multi-vector half-Dslash:
+    links 6 * nrow reals each, 8 per site, or 6 + 2/N3 in temporal gauge (the time links are read only
+    on the slices x3 = 0 / 1); compulsory = each input vector once + each output once; nominal = all 8
+    neighbours of every vector (the paper's count: n 570 / (8 (6 12 + n 9 6)))."""
+    links = (6.0 + 2.0 / N3 if tg else 8.0) * 6 * nrow
+    return links + 12.0 * n, links + 54.0 * n
+
+
+def time_dslash_multi(torch, ctx, fU, fins, fouts, reps=10):
+    for _ in range(2):
+        ctx.qcd_dslash_oe_multi(fU, fouts, fins)
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(reps):
+        ctx.qcd_dslash_oe_multi(fU, fouts, fins)
+    e1.record()
+    torch.cuda.synchronize()
+    return e0.elapsed_time(e1) / reps
+
+
+def variants_sweep(q, torch, ctx, fU_full, dims, peak, nmulti=(1, 2, 3, 4, 6, 8)):
+    """Dslash with the paper's traffic reductions, reported separately from the headline:
+    link storage x temporal gauge x NMULTI.  Throughput does not depend on the link values, so the
+    temporal-gauge rows run on the same links with the field marked (the kernel then skips the time links
+    of x3 != 0); correctness of every variant is tests/test_gpu_variants.py's job."""
+    Vh = int(np.prod(dims)) // 2
+    rsize = 8 if ctx.precision == 64 else 4
+    f12 = ctx.field(q.QCD_GAUGE_2ROW)
+    ctx.qcd_gauge_compress(fU_full, f12)
+    nmax = max(nmulti)
+    fins = [ctx.field(q.QCD_SPINOR_EVEN) for _ in range(nmax)]
+    fouts = [ctx.field(q.QCD_SPINOR_ODD) for _ in range(nmax)]
+    g = torch.Generator(device=ctx.device).manual_seed(7)
+    for f in fins:
+        real = torch.float64 if ctx.precision == 64 else torch.float32
+        f.buf.view(real).copy_(torch.randn(f.buf.numel() // rsize, generator=g, device=ctx.device, dtype=real))
+    rows = []
+    for name, fU, nrow, tg in (("full18", fU_full, 3, 0), ("tworow12", f12, 2, 0), ("tworow12+temporal_gauge", f12, 2, 1)):
+        ctx.qcd_gauge_set_temporal_unit(fU, bool(tg))
+        for n in nmulti:
+            ms = time_dslash_multi(torch, ctx, fU, fins[:n], fouts[:n])
+            comp, nom = variant_reals(nrow, tg, n, dims[3])
+            gbs = comp * rsize * Vh / ms / 1e6
+            rows.append({"links": name, "nmulti": n, "ms": round(ms, 5),
+                         "tflops": round(FLOP_PER_SITE * n * Vh / ms / 1e9, 3),
+                         "gbs_compulsory": round(gbs, 1), "frac_of_measured_copy_peak": round(gbs / peak, 4),
+                         "ai_nominal_flop_per_byte": round(FLOP_PER_SITE * n / (nom * rsize), 3)})
+        ctx.qcd_gauge_set_temporal_unit(fU, False)
+    for f in fins + fouts + [f12]:
+        f.free()
+    return rows
+
+
+def cg_multi_report(q, torch, device, dims, prec, fU_full, m, ns=(1, 2, 4), iters=20):
+    """n CG solves in lock step (qcd_cg_begin_multi / qcd_cg_iterate): ms per iteration and per right-hand side,
+    on the paper's link storage (two rows + temporal gauge marking) and on full links."""
+    rows = []
+    ctx0 = fU_full.ctx
+    for n in ns:
+        ctx = q.Context(dims, prec, device=device, nrhs=n)
+        fb = [ctx.field(q.QCD_SPINOR_EVEN) for _ in range(n)]
+        fx = [ctx.field(q.QCD_SPINOR_EVEN) for _ in range(n)]
+        real = torch.float64 if prec == 64 else torch.float32
+        g = torch.Generator(device=device).manual_seed(11)
+        for f in fb:
+            f.buf.view(real).copy_(torch.randn(f.buf.numel() // (prec // 8), generator=g, device=device, dtype=real))
+        for name, kind in (("full18", q.QCD_GAUGE), ("tworow12+temporal_gauge", q.QCD_GAUGE_2ROW)):
+            if kind == q.QCD_GAUGE:
+                fU = ctx.field(kind, buf=fU_full.buf)      # same device memory, descriptor of the new context
+            else:
+                f12 = ctx0.field(q.QCD_GAUGE_2ROW)
+                ctx0.qcd_gauge_compress(fU_full, f12)
+                fU = ctx.field(kind, buf=f12.buf)
+            ctx.qcd_gauge_set_temporal_unit(fU, kind == q.QCD_GAUGE_2ROW)
+            ctx.qcd_cg_begin_multi(fU, fb, fx, m, 1e-300, 1 << 30)
+            ctx.qcd_cg_iterate(3)
+            torch.cuda.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            ctx.qcd_cg_iterate(iters)
+            e1.record()
+            torch.cuda.synchronize()
+            ctx.qcd_cg_finish_multi()
+            ms = e0.elapsed_time(e1) / iters
+            rows.append({"links": name, "n": n, "ms_per_iter": round(ms, 5), "ms_per_iter_per_rhs": round(ms / n, 5)})
+            fU.free()
+        for f in fb + fx:
+            f.free()
+        ctx.close()
+        torch.cuda.empty_cache()
+    return rows
+
+
 def dslash_report(ms, Vh, rsize, peak):
     comp = REALS_DSLASH_COMPULSORY * rsize * Vh / ms / 1e6
     return {"ms": round(ms, 5), "gflops": round(FLOP_PER_SITE * Vh / ms / 1e6, 1),
@@ -347,17 +442,33 @@ def extras(args, q, torch, ctx, out, cfg, dims, U, b, fU, fb, fx, fo, peak):
                                      f"including the oracle's own set-up; {t_or:.1f} s",
                            "oracle_apply_M_seconds": round(t_true, 2)}
     del x64
+    # ---- variants, reported separately from the headline ----
+    c32 = q.Context(dims, 32, device=ctx.device)
+    gU = c32.field(q.QCD_GAUGE)
+    ctx.qcd_field_convert(gU, fU)                          # fp32 links = round-to-nearest of the fp64 links, on the device
+    gx = c32.field(q.QCD_SPINOR_EVEN)
+    go = c32.field(q.QCD_SPINOR_ODD)
+    # mixed-precision defect-correction CG to the fp64 tolerance (R21)
+    inner_tol = 1e-2
+    mi = ctx.qcd_cg_solve_mixed(c32, fU, gU, fb, fx, gx, c32.field(q.QCD_SPINOR_EVEN), m, cfg["tol64"], inner_tol,
+                                4 * cfg["maxiter"])
+    xm = fx.download()
+    out["cg_mixed"] = {"tol": cfg["tol64"], "inner_tol": inner_tol, "converged": mi["converged"], "outer": mi["outer"],
+                       "inner_iters_fp32": mi["inner_iters"], "m_applications_fp64": mi["m_applications_fp64"],
+                       "s_per_solve": round(mi["seconds"], 4), "true_resid_device_fp64": mi["true_resid"],
+                       "true_resid_oracle_fp64": oracle.true_residual(dims, U, b, xm, m),
+                       "speedup_vs_cg_fp64": round(out["cg_fp64"]["s_per_solve"] / max(mi["seconds"], 1e-9), 3)}
+    del xm
+    out["variants_fp64"] = {"lattice": list(dims), "dslash": variants_sweep(q, torch, ctx, fU, dims, peak)}
+    out["cg_multi_fp64"] = cg_multi_report(q, torch, ctx.device, dims, 64, fU, m)
     # fp32: free the fp64 device fields first
     fU.free(); fb.free(); fx.free(); fo.free()
     ctx.close()
     torch.cuda.empty_cache()
-    c32 = q.Context(dims, 32, device=ctx.device)
     U32, b32 = U.astype(np.complex64), b.astype(np.complex64)
-    gU = c32.field(q.QCD_GAUGE).upload(U32)
     gb = c32.field(q.QCD_SPINOR_EVEN).upload(b32)
-    gx = c32.field(q.QCD_SPINOR_EVEN)
-    go = c32.field(q.QCD_SPINOR_ODD)
     out["dslash_fp32"] = dslash_report(time_dslash(q, torch, c32, gU, gb, go), Vh, 4, peak)
+    out["variants_fp32"] = {"lattice": list(dims), "dslash": variants_sweep(q, torch, c32, gU, dims, peak)}
     if cfg["tol32"]:
         info = c32.qcd_cg_solve(gU, gb, gx, m, cfg["tol32"], cfg["maxiter"])
         x32 = gx.download()
@@ -368,6 +479,20 @@ def extras(args, q, torch, ctx, out, cfg, dims, U, b, fU, fb, fx, fo, peak):
                           "true_resid_oracle_fp64": oracle.true_residual(dims, U32, b32, x32, m),
                           "note": "plain fp32 CG on Haar links stalls in TRUE residual near 1e-4 (DESIGN.md R11)"}
     c32.close()
+    torch.cuda.empty_cache()
+    # the paper's own NMULTI experiment: 32^4, two-row links, temporal gauge (Table 2)
+    if dims == (64, 64, 64, 64):
+        d32 = (32, 32, 32, 32)
+        _, U_32, _ = make_inputs(d32, 2)
+        t2 = {"lattice": list(d32), "paper_A100_tflops": {"fp32": {1: 2.244, 2: 2.532, 3: 2.953, 4: 3.205, 6: 3.090, 8: 3.006},
+                                                           "fp64": {1: 1.245, 2: 1.530, 3: 1.929, 4: 2.199, 6: 2.039, 8: 2.026},
+                                                           "source": "PAPER.md:84-98 Table 2 (A100, OpenCL; other hardware, context only)"}}
+        for prec in (64, 32):
+            c = q.Context(d32, prec, device=ctx.device)
+            f = c.field(q.QCD_GAUGE).upload(U_32)
+            t2[f"fp{prec}"] = variants_sweep(q, torch, c, f, d32, peak)
+            f.free(); c.close()
+        out["variants_table2_32x32x32x32"] = t2
     out["paper_context"] = {"A100_OpenCL_dslash_fp64_TFLOPs_32^4_12real_links_gaugefixed": 1.245,
                             "A100_OpenCL_cg_update_GBs_48^4_fp64": 1351, "source": "PAPER.md:59,87 (other hardware; context only)"}
 

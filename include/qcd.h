@@ -15,7 +15,10 @@
  * Conventions: no factor 1/2; mu = 3 is time;
  * eta_mu(x) = (-1)^{x_0+...+x_{mu-1}}; periodic in mu = 0,1,2, antiperiodic in mu = 3
  * (a hop across the seam x3 = N3-1 <-> 0 carries -1); links are stored as full 3x3
- * complex matrices (18 reals), never modified by the library.
+ * complex matrices (18 reals) in the headline path, never modified by the library.  The
+ * paper's own traffic reductions (two-row links, temporal gauge, several
+ * vectors per link load) and the mixed-precision solver are the calls of the second half
+ * of this header ("Variants"); they are reported separately from the headline.
  *
  * DEVICE LAYOUT ("Structure of Arrays ... all even sites are listed
  * first, followed by all odd sites").  Lattice extents dims = (N0,N1,N2,N3), all even,
@@ -34,6 +37,9 @@
  *            upload reads only the sites of its parity; a half-field download writes
  *            those sites and ZERO on the sites of the other parity.
  *   gauge  : cplx [idx][mu][row][col]      over the full lattice; [idx][mu] = U_{x,mu}.
+ *            The same full 3x3 host layout serves QCD_GAUGE_2ROW (upload keeps rows 0 and 1,
+ *            download reconstructs row 2 = conj(row 0 x row 1)).
+ *   colour matrix : cplx [idx][row][col]   over the full lattice.
  *
  * OWNERSHIP: every device buffer is allocated by the caller (e.g. PyTorch) and only
  * BOUND to a descriptor by qcd_field_alloc; the library never frees caller memory.
@@ -73,7 +79,9 @@ enum {
     QCD_SPINOR_EVEN = 0,   /* 3 planes of Vh cplx, sites of parity 0 */
     QCD_SPINOR_ODD = 1,    /* 3 planes of Vh cplx, sites of parity 1 */
     QCD_SPINOR_FULL = 2,   /* even half-field then odd half-field    */
-    QCD_GAUGE = 3          /* 72 planes of Vh cplx                   */
+    QCD_GAUGE = 3,         /* 72 planes of Vh cplx                   */
+    QCD_GAUGE_2ROW = 4,    /* 48 planes: cplx [parity][mu][k = 3*row + col, row < 2][Vh] */
+    QCD_COLOUR_MATRIX = 5  /* 18 planes: cplx [parity][k = 3*row + col][Vh], one 3x3 matrix per site  */
 };
 
 typedef struct qcd_ctx qcd_ctx;       /* opaque */
@@ -214,6 +222,102 @@ qcd_status qcd_set_dslash_variant(qcd_ctx *ctx, int variant);
 /* Re<a,b> over a half-field pair of the same kind (deterministic two-stage reduction,
  * double accumulation); synchronises.  Used by tests and by callers that need norms. */
 qcd_status qcd_re_dot(qcd_ctx *ctx, const qcd_field *a, const qcd_field *b, double *result);
+
+/* =========================================================================================
+ * Variants: the paper's Dslash optimisations (Sec. 4.3) and mixed precision.
+ * ========================================================================================= */
+
+/* Largest number of vectors one multi-vector call accepts. */
+enum { QCD_MAX_RHS = 8 };
+
+/*
+ * Two-row link storage ("For each link variable, we store only the first two rows,
+ * i.e. 12 floats.  The third row is reconstructed on-the-fly when needed, using the properties
+ * of SU(3) matrices": row2 = conj(row0 x row1)).
+ *   qcd_gauge_compress : U12 (QCD_GAUGE_2ROW) = rows 0, 1 of U (QCD_GAUGE); device to device,
+ *                        asynchronous; carries U's temporal-gauge mark over.
+ * Every operator and solver call of this header accepts a QCD_GAUGE_2ROW field wherever it
+ * accepts a QCD_GAUGE field.  The links must be in SU(3): the reconstruction is exact only then.
+ */
+qcd_status qcd_gauge_compress(qcd_ctx *ctx, const qcd_field *U, qcd_field *U12);
+
+/*
+ * Temporal gauge ("We use gauge fixing to transform the temporal link variables to
+ * 1_{3x3} for all the sites with the temporal coordinate t != 0"; reading R20):
+ *     g(xs,0) = 1,  g(xs,t) = g(xs,t+1) U_{(xs,t),3}^dagger  (t = N3-1 .. 1),
+ *     U'_{x,mu} = g(x) U_{x,mu} g(x+mu)^dagger  =>  U'_{x,3} = 1 for x3 != 0.
+ *   qcd_gauge_fix_temporal : U (QCD_GAUGE) -> U_fixed (QCD_GAUGE, may not alias U) and
+ *                        g (QCD_COLOUR_MATRIX).  U_fixed is MARKED temporal-gauge: kernels
+ *                        applied to it (or to its qcd_gauge_compress copy) do not read the time
+ *                        links of sites with x3 != 0 and use the identity instead.  Asynchronous.
+ *   qcd_gauge_set_temporal_unit : set / clear that mark by hand (for links fixed elsewhere and
+ *                        uploaded; qcd_field_upload clears it).
+ *   qcd_spinor_rotate  : out(x) = g(x) in(x) (dagger = 0) or g(x)^dagger in(x) (dagger = 1) on
+ *                        spinor fields of the same kind; out may alias in.  D[U'] (g phi) =
+ *                        g D[U] phi, so M[U'] x' = g b is solved by x' = g x.
+ */
+qcd_status qcd_gauge_fix_temporal(qcd_ctx *ctx, const qcd_field *U, qcd_field *U_fixed, qcd_field *g);
+qcd_status qcd_gauge_set_temporal_unit(qcd_field *U, int on);
+qcd_status qcd_spinor_rotate(qcd_ctx *ctx, const qcd_field *g, qcd_field *out, const qcd_field *in, int dagger);
+
+/*
+ * Several vectors per link load ("applying D on multiple vectors at once.  This
+ * allows each link variable to be read once and then reused for multiple vectors", NMULTI).
+ *   n    : 1 .. QCD_MAX_RHS
+ *   out, in, b, x, info : HOST arrays of n field pointers / n structs
+ * qcd_dslash_*_multi computes out[i] = D in[i]; qcd_cg_solve_multi runs n INDEPENDENT CG solves
+ * M x[i] = b[i] in lock step (each right-hand side has its own alpha, beta, iteration count and
+ * stop flag on the device and is frozen at its own stopping iteration; result identical to n
+ * calls of qcd_cg_solve).  The workspace must hold qcd_workspace_bytes_multi(ctx, n) bytes.
+ * Returns QCD_OK if every solve converged, else the first non-OK per-solve status
+ * (QCD_ENOTCONVERGED / QCD_EBREAKDOWN); info[i] describes solve i.
+ */
+size_t qcd_workspace_bytes_multi(const qcd_ctx *ctx, int n);
+qcd_status qcd_dslash_eo_multi(qcd_ctx *ctx, const qcd_field *U, int n, qcd_field *const *out_even, const qcd_field *const *in_odd);
+qcd_status qcd_dslash_oe_multi(qcd_ctx *ctx, const qcd_field *U, int n, qcd_field *const *out_odd, const qcd_field *const *in_even);
+qcd_status qcd_cg_solve_multi(qcd_ctx *ctx, const qcd_field *U, int n, const qcd_field *const *b, qcd_field *const *x,
+                              double m, double tol, int maxiter, qcd_cg_info *info);
+/* The multi solve in pieces, as qcd_cg_begin / qcd_cg_iterate / qcd_cg_finish (bench timing). */
+qcd_status qcd_cg_begin_multi(qcd_ctx *ctx, const qcd_field *U, int n, const qcd_field *const *b, qcd_field *const *x,
+                              double m, double tol, int maxiter);
+qcd_status qcd_cg_finish_multi(qcd_ctx *ctx, qcd_cg_info *info);
+
+/*
+ * Precision conversion on the device: dst (a field of a precision-32 context) = round to
+ * nearest of src (same kind, same lattice, precision-64 context), or the widening the other
+ * way.  Both contexts must use the same stream.  Asynchronous.  Carries the temporal-gauge mark.
+ */
+qcd_status qcd_field_convert(qcd_field *dst, const qcd_field *src);
+
+/*
+ * Mixed-precision defect-correction CG (PAPER.md:66 benchmarks CG "in single and double
+ * precision"; reading R21).  Solves M x = b to a TRUE fp64 relative residual <= tol:
+ *     x = 0; r = b
+ *     repeat: rel = |r|/|b|; stop if rel <= tol, or after max_outer corrections, or when the
+ *             inner-iteration budget maxiter is spent
+ *             tol_in = max(inner_tol, 0.5 tol / rel)
+ *             rhs32 = fp32(r / |r|);  e32 = CG_fp32(M[U32], rhs32, tol_in);  x += |r| fp64(e32)
+ *             r = b - M[U64] x                                   (fp64)
+ *   ctx64, ctx32 : contexts of precision 64 and 32 on the same lattice and stream, each with
+ *                  its workspace bound
+ *   U64, U32     : gauge fields of ctx64 / ctx32 (any link storage)
+ *   b, x         : QCD_SPINOR_EVEN fields of ctx64;  x is output only
+ *   rhs32, e32   : QCD_SPINOR_EVEN scratch fields of ctx32
+ *   info         : host pointer, may be NULL
+ * Returns QCD_OK / QCD_ENOTCONVERGED / QCD_EBREAKDOWN / QCD_EINVAL / QCD_ECUDA.  Synchronises.
+ */
+typedef struct qcd_mixed_info {
+    int converged;         /* 1 iff the fp64 residual met tol                                   */
+    int outer;             /* defect-correction steps = inner solves                            */
+    int inner_iters;       /* fp32 CG iterations summed over the inner solves                   */
+    int m_applications_fp64; /* fp64 M applications (one per correction)                        */
+    double true_resid;     /* |b - M x| / |b| in fp64 at exit (computed on the device)          */
+    double seconds;        /* device time of the whole solve                                    */
+} qcd_mixed_info;
+qcd_status qcd_cg_solve_mixed(qcd_ctx *ctx64, qcd_ctx *ctx32, const qcd_field *U64, const qcd_field *U32,
+                              const qcd_field *b, qcd_field *x, qcd_field *rhs32, qcd_field *e32,
+                              double m, double tol, double inner_tol, int maxiter, int max_outer,
+                              qcd_mixed_info *info);
 
 #ifdef __cplusplus
 }

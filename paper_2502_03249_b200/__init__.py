@@ -22,7 +22,8 @@ import numpy as np
 from .build import LIB_PATH
 
 QCD_OK, QCD_EINVAL, QCD_ENOMEM, QCD_ECUDA, QCD_ENOTCONVERGED, QCD_EBREAKDOWN = range(6)
-QCD_SPINOR_EVEN, QCD_SPINOR_ODD, QCD_SPINOR_FULL, QCD_GAUGE = range(4)
+QCD_SPINOR_EVEN, QCD_SPINOR_ODD, QCD_SPINOR_FULL, QCD_GAUGE, QCD_GAUGE_2ROW, QCD_COLOUR_MATRIX = range(6)
+QCD_MAX_RHS = 8
 QCD_K_DSLASH, QCD_K_DSLASH_EPI, QCD_K_UPDATE_XR, QCD_K_UPDATE_P, QCD_K_MISC = range(5)
 
 # every symbol include/qcd.h declares
@@ -33,12 +34,21 @@ SYMBOLS = [
     "qcd_cg_solve", "qcd_cg_begin", "qcd_cg_iterate", "qcd_cg_poll", "qcd_cg_finish",
     "qcd_cg_solve_host", "qcd_profile_enable", "qcd_profile_read", "qcd_launch_count",
     "qcd_set_dslash_variant", "qcd_re_dot",
+    # variants and mixed precision
+    "qcd_gauge_compress", "qcd_gauge_fix_temporal", "qcd_gauge_set_temporal_unit", "qcd_spinor_rotate",
+    "qcd_workspace_bytes_multi", "qcd_dslash_eo_multi", "qcd_dslash_oe_multi", "qcd_cg_solve_multi",
+    "qcd_cg_begin_multi", "qcd_cg_finish_multi", "qcd_field_convert", "qcd_cg_solve_mixed",
 ]
 
 
 class qcd_cg_info(ctypes.Structure):
     _fields_ = [("iters", ctypes.c_int), ("converged", ctypes.c_int), ("rel_resid", ctypes.c_double),
                 ("bnorm2", ctypes.c_double), ("seconds", ctypes.c_double)]
+
+
+class qcd_mixed_info(ctypes.Structure):
+    _fields_ = [("converged", ctypes.c_int), ("outer", ctypes.c_int), ("inner_iters", ctypes.c_int),
+                ("m_applications_fp64", ctypes.c_int), ("true_resid", ctypes.c_double), ("seconds", ctypes.c_double)]
 
 
 class QcdError(RuntimeError):
@@ -87,6 +97,18 @@ def load_library() -> ctypes.CDLL:
         "qcd_launch_count": (ctypes.c_longlong, [vp]),
         "qcd_set_dslash_variant": (ci, [vp, ci]),
         "qcd_re_dot": (ci, [vp, vp, vp, P(cd)]),
+        "qcd_gauge_compress": (ci, [vp, vp, vp]),
+        "qcd_gauge_fix_temporal": (ci, [vp, vp, vp, vp]),
+        "qcd_gauge_set_temporal_unit": (ci, [vp, ci]),
+        "qcd_spinor_rotate": (ci, [vp, vp, vp, vp, ci]),
+        "qcd_workspace_bytes_multi": (sz, [vp, ci]),
+        "qcd_dslash_eo_multi": (ci, [vp, vp, ci, P(vp), P(vp)]),
+        "qcd_dslash_oe_multi": (ci, [vp, vp, ci, P(vp), P(vp)]),
+        "qcd_cg_solve_multi": (ci, [vp, vp, ci, P(vp), P(vp), cd, cd, ci, P(qcd_cg_info)]),
+        "qcd_cg_begin_multi": (ci, [vp, vp, ci, P(vp), P(vp), cd, cd, ci]),
+        "qcd_cg_finish_multi": (ci, [vp, P(qcd_cg_info)]),
+        "qcd_field_convert": (ci, [vp, vp]),
+        "qcd_cg_solve_mixed": (ci, [vp, vp, vp, vp, vp, vp, vp, vp, cd, cd, cd, ci, ci, P(qcd_mixed_info)]),
     }
     for name, (res, args) in sig.items():
         fn = getattr(lib, name)
@@ -105,11 +127,15 @@ def _torch():
 class Field:
     """A caller-owned torch uint8 device buffer bound to a qcd_field descriptor."""
 
-    def __init__(self, ctx: "Context", kind: int):
+    def __init__(self, ctx: "Context", kind: int, buf=None):
+        """buf: an existing uint8 device tensor to bind (e.g. the links of another context on the same
+        lattice and precision: qcd_field_alloc only binds, so descriptors may share memory)."""
         torch = _torch()
         self.ctx, self.kind = ctx, kind
         self.nbytes = ctx.qcd_field_bytes(kind)
-        self.buf = torch.empty(self.nbytes, dtype=torch.uint8, device=ctx.device)
+        if buf is None:
+            buf = torch.empty(self.nbytes, dtype=torch.uint8, device=ctx.device)
+        self.buf = buf
         h = ctypes.c_void_p()
         ctx._check(ctx.lib.qcd_field_alloc(ctx.handle, kind, ctypes.c_void_p(self.buf.data_ptr()), self.nbytes,
                                             ctypes.byref(h)), "qcd_field_alloc")
@@ -117,7 +143,9 @@ class Field:
 
     def host_shape(self):
         v = self.ctx.volume
-        return (v, 4, 3, 3) if self.kind == QCD_GAUGE else (v, 3)
+        if self.kind in (QCD_GAUGE, QCD_GAUGE_2ROW):
+            return (v, 4, 3, 3)
+        return (v, 3, 3) if self.kind == QCD_COLOUR_MATRIX else (v, 3)
 
     def upload(self, host: np.ndarray) -> "Field":
         """qcd_field_upload: host array in the canonical layout, complex dtype of the context precision."""
@@ -150,7 +178,7 @@ class Field:
 class Context:
     """qcd_ctx plus the torch-owned workspace.  Methods carry the C names and marshal only."""
 
-    def __init__(self, dims, precision: int = 64, stream=None, device="cuda:0", workspace: bool = True):
+    def __init__(self, dims, precision: int = 64, stream=None, device="cuda:0", workspace: bool = True, nrhs: int = 1):
         torch = _torch()
         self.lib = load_library()
         self.dims = tuple(int(d) for d in dims)
@@ -168,7 +196,7 @@ class Context:
         self.volume = self.dims[0] * self.dims[1] * self.dims[2] * self.dims[3]
         self.ws = None
         if workspace:
-            self.ws = torch.empty(self.qcd_workspace_bytes(), dtype=torch.uint8, device=self.device)
+            self.ws = torch.empty(self.qcd_workspace_bytes_multi(nrhs), dtype=torch.uint8, device=self.device)
             self._check(self.lib.qcd_set_workspace(self.handle, ctypes.c_void_p(self.ws.data_ptr()), self.ws.numel()),
                         "qcd_set_workspace")
 
@@ -178,8 +206,8 @@ class Context:
             raise QcdError(st, where, self.lib.qcd_last_error(self.handle).decode())
         return st
 
-    def field(self, kind: int) -> Field:
-        return Field(self, kind)
+    def field(self, kind: int, buf=None) -> Field:
+        return Field(self, kind, buf)
 
     def close(self):
         if self.handle:
@@ -266,3 +294,63 @@ class Context:
         r = ctypes.c_double()
         self._check(self.lib.qcd_re_dot(self.handle, a.handle, b.handle, ctypes.byref(r)), "qcd_re_dot")
         return r.value
+
+    # ---- variants -------------------------------------------------------
+    @staticmethod
+    def _handles(fields):
+        return (ctypes.c_void_p * len(fields))(*[f.handle.value for f in fields])
+
+    def qcd_workspace_bytes_multi(self, n: int) -> int:
+        return int(self.lib.qcd_workspace_bytes_multi(self.handle, int(n)))
+
+    def qcd_gauge_compress(self, U: Field, U12: Field):
+        self._check(self.lib.qcd_gauge_compress(self.handle, U.handle, U12.handle), "qcd_gauge_compress")
+
+    def qcd_gauge_fix_temporal(self, U: Field, U_fixed: Field, g: Field):
+        self._check(self.lib.qcd_gauge_fix_temporal(self.handle, U.handle, U_fixed.handle, g.handle), "qcd_gauge_fix_temporal")
+
+    def qcd_gauge_set_temporal_unit(self, U: Field, on: bool):
+        self._check(self.lib.qcd_gauge_set_temporal_unit(U.handle, 1 if on else 0), "qcd_gauge_set_temporal_unit")
+
+    def qcd_spinor_rotate(self, g: Field, out: Field, in_: Field, dagger: bool = False):
+        self._check(self.lib.qcd_spinor_rotate(self.handle, g.handle, out.handle, in_.handle, 1 if dagger else 0), "qcd_spinor_rotate")
+
+    def qcd_dslash_eo_multi(self, U: Field, out_even, in_odd):
+        self._check(self.lib.qcd_dslash_eo_multi(self.handle, U.handle, len(out_even), self._handles(out_even),
+                                                 self._handles(in_odd)), "qcd_dslash_eo_multi")
+
+    def qcd_dslash_oe_multi(self, U: Field, out_odd, in_even):
+        self._check(self.lib.qcd_dslash_oe_multi(self.handle, U.handle, len(out_odd), self._handles(out_odd),
+                                                 self._handles(in_even)), "qcd_dslash_oe_multi")
+
+    def qcd_cg_solve_multi(self, U: Field, b, x, m: float, tol: float, maxiter: int):
+        n = len(b)
+        infos = (qcd_cg_info * n)()
+        st = self._check(self.lib.qcd_cg_solve_multi(self.handle, U.handle, n, self._handles(b), self._handles(x),
+                                                     float(m), float(tol), int(maxiter), infos), "qcd_cg_solve_multi", self._CG_OK)
+        return [self._info(infos[i], st) for i in range(n)]
+
+    def qcd_cg_begin_multi(self, U: Field, b, x, m: float, tol: float, maxiter: int):
+        self._multi_n = len(b)
+        self._check(self.lib.qcd_cg_begin_multi(self.handle, U.handle, len(b), self._handles(b), self._handles(x),
+                                                float(m), float(tol), int(maxiter)), "qcd_cg_begin_multi")
+
+    def qcd_cg_finish_multi(self):
+        n = self._multi_n
+        infos = (qcd_cg_info * n)()
+        st = self._check(self.lib.qcd_cg_finish_multi(self.handle, infos), "qcd_cg_finish_multi", self._CG_OK)
+        return [self._info(infos[i], st) for i in range(n)]
+
+    def qcd_field_convert(self, dst: Field, src: Field):
+        """dst and src belong to two contexts of different precision on the same lattice and stream."""
+        dst.ctx._check(self.lib.qcd_field_convert(dst.handle, src.handle), "qcd_field_convert")
+
+    def qcd_cg_solve_mixed(self, ctx32: "Context", U64: Field, U32: Field, b: Field, x: Field, rhs32: Field, e32: Field,
+                           m: float, tol: float, inner_tol: float, maxiter: int, max_outer: int = 50) -> dict:
+        i = qcd_mixed_info()
+        st = self._check(self.lib.qcd_cg_solve_mixed(self.handle, ctx32.handle, U64.handle, U32.handle, b.handle, x.handle,
+                                                     rhs32.handle, e32.handle, float(m), float(tol), float(inner_tol),
+                                                     int(maxiter), int(max_outer), ctypes.byref(i)),
+                         "qcd_cg_solve_mixed", self._CG_OK)
+        return dict(status=st, converged=bool(i.converged), outer=i.outer, inner_iters=i.inner_iters,
+                    m_applications_fp64=i.m_applications_fp64, true_resid=i.true_resid, seconds=i.seconds)

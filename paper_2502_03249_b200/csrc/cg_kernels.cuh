@@ -9,6 +9,10 @@
 //   cg_update_p  : p = r + beta p
 //   re_dot       : Re<a,b>
 //
+// Several right-hand sides (NMULTI) are independent solves: blockIdx.y is the
+// right-hand side, each with its own CgScalars entry, partials row and ticket; r, p, Ap are
+// [nrhs][half-field] in the workspace, x and b are the caller's fields (RhsPtrs).
+//
 // Field arithmetic is in T; products for the reductions are formed and summed in double
 // (reading R9); alpha, beta are rounded to T before they multiply a field.
 #pragma once
@@ -43,13 +47,24 @@ __device__ __forceinline__ void vxpay(float4 &a, float s, const float4 &b)
 
 enum { BLAS_BLOCK = 256, BLAS_ITEMS = 4 };
 
+template <typename V>
+struct RhsPtrs {
+    V *x[MAXRHS];
+    const V *b[MAXRHS];
+};
+
 template <typename T>
 __global__ void __launch_bounds__(BLAS_BLOCK) cg_init_kernel(
-    int n16, const typename Vec16<T>::type *__restrict__ b, typename Vec16<T>::type *__restrict__ x,
+    int n16, const RhsPtrs<typename Vec16<T>::type> ptrs,
     typename Vec16<T>::type *__restrict__ r, typename Vec16<T>::type *__restrict__ p,
     double tol, int maxiter, double *partials, CgScalars *scal)
 {
     typedef typename Vec16<T>::type V;
+    const int rhs = blockIdx.y;
+    const V *__restrict__ b = ptrs.b[rhs];
+    V *__restrict__ x = ptrs.x[rhs];
+    r += (size_t)rhs * n16; p += (size_t)rhs * n16;
+    partials += (size_t)rhs * gridDim.x; scal += rhs;
     double s = 0.0;
     const int base = blockIdx.x * (BLAS_BLOCK * BLAS_ITEMS) + threadIdx.x;
     V vb[BLAS_ITEMS];
@@ -86,12 +101,17 @@ __global__ void __launch_bounds__(BLAS_BLOCK) cg_init_kernel(
 
 template <typename T>
 __global__ void __launch_bounds__(BLAS_BLOCK) cg_update_xr_kernel(
-    int n16, typename Vec16<T>::type *__restrict__ x, typename Vec16<T>::type *__restrict__ r,
+    int n16, const RhsPtrs<typename Vec16<T>::type> ptrs, typename Vec16<T>::type *__restrict__ r,
     const typename Vec16<T>::type *__restrict__ p, const typename Vec16<T>::type *__restrict__ Ap,
     double *partials, CgScalars *scal)
 {
     typedef typename Vec16<T>::type V;
+    const int rhs = blockIdx.y;
+    scal += rhs;
     if (scal->flag != 0) return;
+    V *__restrict__ x = ptrs.x[rhs];
+    r += (size_t)rhs * n16; p += (size_t)rhs * n16; Ap += (size_t)rhs * n16;
+    partials += (size_t)rhs * gridDim.x;
     const T alpha = (T)scal->alpha;
     double s = 0.0;
     const int base = blockIdx.x * (BLAS_BLOCK * BLAS_ITEMS) + threadIdx.x;
@@ -133,7 +153,10 @@ __global__ void __launch_bounds__(BLAS_BLOCK) cg_update_p_kernel(
     const CgScalars *scal)
 {
     typedef typename Vec16<T>::type V;
+    const int rhs = blockIdx.y;
+    scal += rhs;
     if (scal->flag != 0) return;
+    p += (size_t)rhs * n16; r += (size_t)rhs * n16;
     const T beta = (T)scal->beta;
     const int base = blockIdx.x * (BLAS_BLOCK * BLAS_ITEMS) + threadIdx.x;
     V vp[BLAS_ITEMS], vr[BLAS_ITEMS];

@@ -14,25 +14,33 @@
 // MODE 1: out = m^2 v - D phi                           (qcd_apply_M, second half)
 // MODE 2: MODE 1 + block partial of Re<v,out> and the CG alpha step in the last block
 //         ("epilogue fused into the D_eo kernel")
+//
+// The paper's own traffic reductions are template parameters of the same kernel:
+// NROW = 2 : "we store only the first two rows, i.e. 12 floats.  The third row is reconstructed
+//            on-the-fly ... using the properties of SU(3) matrices": row2 = conj(row0 x row1)
+// TG = 1   : "gauge fixing to transform the temporal link variables to 1 for all the sites with
+//            the temporal coordinate t != 0": time links with t != 0 are not loaded at all
+// NRHS = n : "applying D on multiple vectors at once ... each link variable to be read once and
+//            then reused for multiple vectors" (NMULTI)
 #pragma once
 #include "lattice.cuh"
 #include "reduce.cuh"
 
 namespace qcd {
 
-template <typename T>
+template <typename T, int NRHS>
 struct DslashArgs {
     typedef typename Cplx<T>::type C;
     Lattice L;
     int parity;            // parity of the OUTPUT sites (0: D_eo, 1: D_oe)
-    const C *U;            // gauge field, 72 planes
-    const C *in;           // half-field of parity 1-parity, 3 planes
-    C *out;                // half-field of parity `parity`, 3 planes
-    const C *v;            // MODE >= 1: half-field of parity `parity`
+    const C *U;            // gauge field, 2 x 4 x (3 NROW) planes
+    const C *in[NRHS];     // half-fields of parity 1-parity, 3 planes each
+    C *out[NRHS];          // half-fields of parity `parity`, 3 planes each
+    const C *v[NRHS];      // MODE >= 1: half-fields of parity `parity`
     T m2;                  // MODE >= 1
-    double *partials;      // MODE 2
-    CgScalars *scal;       // MODE 2 (and flag source when check_flag)
-    int check_flag;        // return immediately when scal->flag != 0 (CG no-op iterations)
+    double *partials;      // MODE 2: [NRHS][gridDim.x]
+    CgScalars *scal;       // MODE 2: NRHS entries (and flag source when check_flag)
+    int check_flag;        // return immediately when every scal[r].flag != 0 (CG no-op iterations)
 };
 
 // acc += U * p
@@ -68,76 +76,171 @@ __device__ __forceinline__ void matdag_vec_acc(C acc[3], const C u[9], const C p
     }
 }
 
-template <typename T, int MODE, int BLOCK, int MINB>
-__global__ void __launch_bounds__(BLOCK, MINB) dslash_kernel(const DslashArgs<T> a)
+// conj(a * b - c * d)
+template <typename C>
+__device__ __forceinline__ C conj_cross(const C &a, const C &b, const C &c, const C &d)
+{
+    C r;
+    r.x = a.x * b.x - a.y * b.y - c.x * d.x + c.y * d.y;
+    r.y = -(a.x * b.y + a.y * b.x - c.x * d.y - c.y * d.x);
+    return r;
+}
+
+// Third row of an SU(3) matrix from its first two: rows are orthonormal and
+// det = 1, hence row2 = conj(row0 x row1).
+template <typename C>
+__device__ __forceinline__ void reconstruct_third_row(C u[9])
+{
+    u[6] = conj_cross(u[1], u[5], u[2], u[4]);
+    u[7] = conj_cross(u[2], u[3], u[0], u[5]);
+    u[8] = conj_cross(u[0], u[4], u[1], u[3]);
+}
+
+// One link = 3 NROW planes, Vh apart.
+template <int NROW, typename C>
+__device__ __forceinline__ void load_link(C u[9], const C *p, size_t Vh, uint64_t pol)
+{
+#pragma unroll
+    for (int k = 0; k < 3 * NROW; ++k) u[k] = ld_stream(p + (size_t)k * Vh, pol);
+}
+
+template <typename T, typename C>
+__device__ __forceinline__ void load_spinor(C p[3], const C *f, size_t Vh, int site, T sign, uint64_t pol)
+{
+#pragma unroll
+    for (int c = 0; c < 3; ++c) p[c] = ld_keep(f + (size_t)c * Vh + site, pol);
+#pragma unroll
+    for (int c = 0; c < 3; ++c) { p[c].x *= sign; p[c].y *= sign; }     // exact: sign is +-1
+}
+
+template <typename C>
+__device__ __forceinline__ void vec_acc(C acc[3], const C p[3])
+{
+#pragma unroll
+    for (int c = 0; c < 3; ++c) { acc[c].x += p[c].x; acc[c].y += p[c].y; }
+}
+
+template <typename T, int MODE, int NROW, int TG, int NRHS, int BLOCK, int MINB>
+__global__ void __launch_bounds__(BLOCK, MINB) dslash_kernel(const DslashArgs<T, NRHS> a)
 {
     typedef typename Cplx<T>::type C;
-    if (a.check_flag && a.scal->flag != 0) return;
+    if (a.check_flag) {
+        bool all_done = true;
+#pragma unroll
+        for (int r = 0; r < NRHS; ++r) all_done = all_done && (a.scal[r].flag != 0);
+        if (all_done) return;
+    }
 
     const int cb = blockIdx.x * BLOCK + threadIdx.x;
     const bool active = cb < a.L.Vh;
     const size_t Vh = (size_t)a.L.Vh;
-    double dot = 0.0;
+    double dot[NRHS];
+#pragma unroll
+    for (int r = 0; r < NRHS; ++r) dot[r] = 0.0;
 
     if (active) {
         const SiteGeom g = site_geometry(a.L, a.parity, cb);
         const uint64_t pol_stream = l2_policy_evict_first();
         const uint64_t pol_keep = l2_policy_evict_last();
-        const C *Uf = a.U + (size_t)(a.parity * 36) * Vh + cb;          // U_{x,mu}: own parity block
-        const C *Ub = a.U + (size_t)((1 - a.parity) * 36) * Vh;         // U_{x-mu,mu}: other parity block
+        const C *Uf = a.U + (size_t)(a.parity * 12 * NROW) * Vh + cb;          // U_{x,mu}: own parity block
+        const C *Ub = a.U + (size_t)((1 - a.parity) * 12 * NROW) * Vh;         // U_{x-mu,mu}: other parity block
 
-        C acc[3];
-        acc[0].x = acc[0].y = acc[1].x = acc[1].y = acc[2].x = acc[2].y = (T)0;
+        C acc[NRHS][3];
+#pragma unroll
+        for (int r = 0; r < NRHS; ++r)
+            acc[r][0].x = acc[r][0].y = acc[r][1].x = acc[r][1].y = acc[r][2].x = acc[r][2].y = (T)0;
 
 #pragma unroll
         for (int mu = 0; mu < 4; ++mu) {
-            C uf[9], ub[9], pf[3], pb[3];
-            const C *ufp = Uf + (size_t)(mu * 9) * Vh;
-            const C *ubp = Ub + (size_t)(mu * 9) * Vh + g.nb[mu];
-#pragma unroll
-            for (int k = 0; k < 9; ++k) uf[k] = ld_stream(ufp + (size_t)k * Vh, pol_stream);
-#pragma unroll
-            for (int k = 0; k < 9; ++k) ub[k] = ld_stream(ubp + (size_t)k * Vh, pol_stream);
-#pragma unroll
-            for (int c = 0; c < 3; ++c) pf[c] = ld_keep(a.in + (size_t)c * Vh + g.nf[mu], pol_keep);
-#pragma unroll
-            for (int c = 0; c < 3; ++c) pb[c] = ld_keep(a.in + (size_t)c * Vh + g.nb[mu], pol_keep);
+            const C *ufp = Uf + (size_t)(mu * 3 * NROW) * Vh;
+            const C *ubp = Ub + (size_t)(mu * 3 * NROW) * Vh + g.nb[mu];
             const T sf = (T)g.sf[mu], sb = (T)g.sb[mu];
+            // temporal gauge: U_{x,3} = 1 unless x3 == 0; U_{x-3,3} = 1 unless x3 - 1 == 0
+            const bool unit_f = TG && mu == 3 && g.x3 != 0;
+            const bool unit_b = TG && mu == 3 && g.x3 != 1;
+
+            if (NRHS <= 2 && !(TG && mu == 3)) {
+                // every load of this direction is issued before its first use
+                C uf[9], ub[9], pf[NRHS][3], pb[NRHS][3];
+                load_link<NROW, C>(uf, ufp, Vh, pol_stream);
+                load_link<NROW, C>(ub, ubp, Vh, pol_stream);
 #pragma unroll
-            for (int c = 0; c < 3; ++c) {
-                pf[c].x *= sf; pf[c].y *= sf;     // exact: sf, sb are +-1
-                pb[c].x *= sb; pb[c].y *= sb;
+                for (int r = 0; r < NRHS; ++r) load_spinor<T, C>(pf[r], a.in[r], Vh, g.nf[mu], sf, pol_keep);
+#pragma unroll
+                for (int r = 0; r < NRHS; ++r) load_spinor<T, C>(pb[r], a.in[r], Vh, g.nb[mu], sb, pol_keep);
+                if (NROW == 2) { reconstruct_third_row<C>(uf); reconstruct_third_row<C>(ub); }
+#pragma unroll
+                for (int r = 0; r < NRHS; ++r) {
+                    mat_vec_acc<T, C>(acc[r], uf, pf[r]);
+                    matdag_vec_acc<T, C>(acc[r], ub, pb[r]);
+                }
+            } else {
+                // forward hop then backward hop: one link in registers, reused by every vector
+                {
+                    C u[9], p[NRHS][3];
+                    if (!unit_f) load_link<NROW, C>(u, ufp, Vh, pol_stream);
+#pragma unroll
+                    for (int r = 0; r < NRHS; ++r) load_spinor<T, C>(p[r], a.in[r], Vh, g.nf[mu], sf, pol_keep);
+                    if (!unit_f) {
+                        if (NROW == 2) reconstruct_third_row<C>(u);
+#pragma unroll
+                        for (int r = 0; r < NRHS; ++r) mat_vec_acc<T, C>(acc[r], u, p[r]);
+                    } else {
+#pragma unroll
+                        for (int r = 0; r < NRHS; ++r) vec_acc<C>(acc[r], p[r]);
+                    }
+                }
+                {
+                    C u[9], p[NRHS][3];
+                    if (!unit_b) load_link<NROW, C>(u, ubp, Vh, pol_stream);
+#pragma unroll
+                    for (int r = 0; r < NRHS; ++r) load_spinor<T, C>(p[r], a.in[r], Vh, g.nb[mu], sb, pol_keep);
+                    if (!unit_b) {
+                        if (NROW == 2) reconstruct_third_row<C>(u);
+#pragma unroll
+                        for (int r = 0; r < NRHS; ++r) matdag_vec_acc<T, C>(acc[r], u, p[r]);
+                    } else {
+#pragma unroll
+                        for (int r = 0; r < NRHS; ++r) vec_acc<C>(acc[r], p[r]);
+                    }
+                }
             }
-            mat_vec_acc<T, C>(acc, uf, pf);
-            matdag_vec_acc<T, C>(acc, ub, pb);
         }
 
-        if (MODE >= 1) {
 #pragma unroll
-            for (int c = 0; c < 3; ++c) {
-                const C vv = a.v[(size_t)c * Vh + cb];
-                C o;
-                o.x = fma(a.m2, vv.x, -acc[c].x);
-                o.y = fma(a.m2, vv.y, -acc[c].y);
-                a.out[(size_t)c * Vh + cb] = o;
-                if (MODE == 2) dot += (double)vv.x * (double)o.x + (double)vv.y * (double)o.y;
+        for (int r = 0; r < NRHS; ++r) {
+            if (MODE >= 1) {
+#pragma unroll
+                for (int c = 0; c < 3; ++c) {
+                    const C vv = a.v[r][(size_t)c * Vh + cb];
+                    C o;
+                    o.x = fma(a.m2, vv.x, -acc[r][c].x);
+                    o.y = fma(a.m2, vv.y, -acc[r][c].y);
+                    a.out[r][(size_t)c * Vh + cb] = o;
+                    if (MODE == 2) dot[r] += (double)vv.x * (double)o.x + (double)vv.y * (double)o.y;
+                }
+            } else {
+#pragma unroll
+                for (int c = 0; c < 3; ++c) a.out[r][(size_t)c * Vh + cb] = acc[r][c];
             }
-        } else {
-#pragma unroll
-            for (int c = 0; c < 3; ++c) a.out[(size_t)c * Vh + cb] = acc[c];
         }
     }
 
     if (MODE == 2) {
-        __shared__ double smem[BLOCK / 32];
+        __shared__ double smem[NRHS * (BLOCK / 32)];
         __shared__ int last;
-        if (publish_partial<BLOCK>(dot, a.partials, &a.scal->ticket, smem, &last)) {
-            const double pAp = final_sum<BLOCK>(a.partials, (int)gridDim.x, smem);
-            if (threadIdx.x == 0) {
-                CgScalars *s = a.scal;
-                s->pAp = pAp;
-                if (!(pAp > 0.0)) s->flag = 3;          // breakdown: <p,Mp> <= 0 or NaN
-                else s->alpha = s->rr / pAp;
+        if (publish_partials<BLOCK, NRHS>(dot, a.partials, (size_t)gridDim.x, &a.scal[0].ticket, smem, &last)) {
+            for (int r = 0; r < NRHS; ++r) {
+                const double pAp = final_sum<BLOCK>(a.partials + (size_t)r * gridDim.x, (int)gridDim.x, smem);
+                if (threadIdx.x == 0) {
+                    CgScalars *s = a.scal + r;
+                    if (s->flag == 0) {
+                        s->pAp = pAp;
+                        if (!(pAp > 0.0)) s->flag = 3;          // breakdown: <p,Mp> <= 0 or NaN
+                        else s->alpha = s->rr / pAp;
+                    }
+                }
+                __syncthreads();
             }
         }
     }

@@ -1,0 +1,87 @@
+// Dispatch from a runtime DslashLaunch to one instantiation of dslash_kernel.  Included by the
+// four dslash_*.cu translation units, each of which instantiates launch_dslash_impl once.
+#pragma once
+#include "dslash.cuh"
+#include "dslash_launch.h"
+
+namespace qcd {
+
+// Block shape per (precision, NRHS): 128 threads; the minimum resident blocks per SM fixes the
+// register cap (65536 / (128 * MINB)): accumulators grow by 6 reals per extra vector.
+template <typename T, int NRHS> struct DslashCfg;
+template <> struct DslashCfg<double, 1> { enum { BLOCK = 128, MINB = 4 }; };
+template <> struct DslashCfg<double, 2> { enum { BLOCK = 128, MINB = 3 }; };
+template <> struct DslashCfg<double, 3> { enum { BLOCK = 128, MINB = 2 }; };
+template <> struct DslashCfg<double, 4> { enum { BLOCK = 128, MINB = 2 }; };
+template <> struct DslashCfg<double, 5> { enum { BLOCK = 128, MINB = 2 }; };
+template <> struct DslashCfg<double, 6> { enum { BLOCK = 128, MINB = 2 }; };
+template <> struct DslashCfg<double, 7> { enum { BLOCK = 128, MINB = 2 }; };
+template <> struct DslashCfg<double, 8> { enum { BLOCK = 128, MINB = 2 }; };
+template <> struct DslashCfg<float, 1> { enum { BLOCK = 128, MINB = 4 }; };
+template <> struct DslashCfg<float, 2> { enum { BLOCK = 128, MINB = 4 }; };
+template <> struct DslashCfg<float, 3> { enum { BLOCK = 128, MINB = 4 }; };
+template <> struct DslashCfg<float, 4> { enum { BLOCK = 128, MINB = 3 }; };
+template <> struct DslashCfg<float, 5> { enum { BLOCK = 128, MINB = 3 }; };
+template <> struct DslashCfg<float, 6> { enum { BLOCK = 128, MINB = 3 }; };
+template <> struct DslashCfg<float, 7> { enum { BLOCK = 128, MINB = 2 }; };
+template <> struct DslashCfg<float, 8> { enum { BLOCK = 128, MINB = 2 }; };
+
+template <typename T, int MODE, int NROW, int TG, int NRHS, int BLOCK, int MINB>
+static cudaError_t launch_cfg(const DslashLaunch &d)
+{
+    typedef typename Cplx<T>::type C;
+    DslashArgs<T, NRHS> a;
+    a.L = d.L; a.parity = d.parity; a.U = (const C *)d.U;
+    for (int r = 0; r < NRHS; ++r) { a.in[r] = (const C *)d.in[r]; a.out[r] = (C *)d.out[r]; a.v[r] = (const C *)d.v[r]; }
+    a.m2 = (T)d.m2; a.partials = d.partials; a.scal = d.scal; a.check_flag = d.check_flag;
+    const int grid = (d.L.Vh + BLOCK - 1) / BLOCK;
+    dslash_kernel<T, MODE, NROW, TG, NRHS, BLOCK, MINB><<<grid, BLOCK, 0, d.stream>>>(a);
+    return cudaGetLastError();
+}
+
+template <typename T, int MODE, int NROW, int TG, int NRHS>
+static cudaError_t launch_nrhs(const DslashLaunch &d)
+{
+    if constexpr (NRHS == 1 && TG == 0) {
+        switch (d.variant) {       // block-shape sweep of the headline kernel
+        case 1: return launch_cfg<T, MODE, NROW, TG, 1, 64, 8>(d);
+        case 2: return launch_cfg<T, MODE, NROW, TG, 1, 256, 2>(d);
+        case 3: return launch_cfg<T, MODE, NROW, TG, 1, 128, 3>(d);
+        default: break;
+        }
+    }
+    return launch_cfg<T, MODE, NROW, TG, NRHS, DslashCfg<T, NRHS>::BLOCK, DslashCfg<T, NRHS>::MINB>(d);
+}
+
+template <typename T, int MODE, int NROW, int TG>
+static cudaError_t launch_tg(const DslashLaunch &d)
+{
+    if constexpr (MODE == 1) return d.nrhs == 1 ? launch_nrhs<T, MODE, NROW, TG, 1>(d) : cudaErrorInvalidValue;
+    else switch (d.nrhs) {
+    case 1: return launch_nrhs<T, MODE, NROW, TG, 1>(d);
+    case 2: return launch_nrhs<T, MODE, NROW, TG, 2>(d);
+    case 3: return launch_nrhs<T, MODE, NROW, TG, 3>(d);
+    case 4: return launch_nrhs<T, MODE, NROW, TG, 4>(d);
+    case 5: return launch_nrhs<T, MODE, NROW, TG, 5>(d);
+    case 6: return launch_nrhs<T, MODE, NROW, TG, 6>(d);
+    case 7: return launch_nrhs<T, MODE, NROW, TG, 7>(d);
+    case 8: return launch_nrhs<T, MODE, NROW, TG, 8>(d);
+    default: return cudaErrorInvalidValue;
+    }
+}
+
+template <typename T, int NROW>
+static cudaError_t launch_dslash_impl(const DslashLaunch &d)
+{
+    switch (d.mode * 2 + (d.tg ? 1 : 0)) {
+    case 0: return launch_tg<T, 0, NROW, 0>(d);
+    case 1: return launch_tg<T, 0, NROW, 1>(d);
+    case 2: return launch_tg<T, 1, NROW, 0>(d);
+    case 3: return launch_tg<T, 1, NROW, 1>(d);
+    case 4: return launch_tg<T, 2, NROW, 0>(d);
+    case 5: return launch_tg<T, 2, NROW, 1>(d);
+    default: return cudaErrorInvalidValue;
+    }
+}
+
+} // namespace qcd

@@ -88,6 +88,7 @@ __device__ __forceinline__ float4 ld_keep(const float4 *p, uint64_t pol)
 struct SiteGeom {
     int nf[4], nb[4];   // cb of x+mu, x-mu
     float sf[4], sb[4]; // eta_mu(x) * seam sign of the forward hop ; MINUS eta_mu(x-mu) * seam sign of the backward hop
+    int x3;             // time coordinate (temporal-gauge kernels: which time links are the identity)
 };
 
 __device__ __forceinline__ SiteGeom site_geometry(const Lattice &L, int parity, int cb)
@@ -122,6 +123,7 @@ __device__ __forceinline__ SiteGeom site_geometry(const Lattice &L, int parity, 
     g.sf[2] = e2;   g.sb[2] = -e2;
     g.sf[3] = (x3 + 1 == L.N3) ? -e3 : e3;           // forward hop across the time seam
     g.sb[3] = (x3 == 0) ? e3 : -e3;                  // backward hop across the time seam
+    g.x3 = x3;
     return g;
 }
 

@@ -15,9 +15,11 @@
 #include <string>
 
 #include "cg_kernels.cuh"
-#include "dslash.cuh"
+#include "dslash_launch.h"
+#include "gauge_kernels.cuh"
 #include "lattice.cuh"
 #include "layout_kernels.cuh"
+#include "mixed_kernels.cuh"
 #include "reduce.cuh"
 
 using namespace qcd;
@@ -32,12 +34,15 @@ struct qcd_field {
     int kind;
     void *ptr;
     size_t nbytes;
+    int tg;                   // gauge fields: time links with x3 != 0 are the identity (temporal gauge)
 };
 
 struct CgState {
     bool active;
-    const qcd_field *U, *b;
-    qcd_field *x;
+    int n;                    // right-hand sides solved in lock step
+    const qcd_field *U;
+    const void *b[MAXRHS];
+    void *x[MAXRHS];
     double m, tol;
     int maxiter;
     cudaEvent_t ev_begin, ev_end;
@@ -48,11 +53,11 @@ struct qcd_ctx {
     int prec;                 // 64 or 32
     size_t rsize;             // sizeof(real)
     cudaStream_t stream;
-    CgScalars *d_scal;        // CG recurrence state
-    CgScalars *d_aux;         // scratch state for qcd_apply_M / qcd_re_dot
+    CgScalars *d_scal;        // CG recurrence state, MAXRHS entries
+    CgScalars *d_aux;         // scratch state for qcd_apply_M / qcd_re_dot / the mixed solver
     double *d_partials;       // stage-1 partial sums
     int partials_cap;
-    CgScalars *h_scal;        // pinned, POLL_SLOTS entries
+    CgScalars *h_scal;        // pinned, POLL_SLOTS x MAXRHS entries
     cudaEvent_t poll_ev[POLL_SLOTS];
     void *d_stage;
     void *ws;
@@ -110,11 +115,18 @@ extern "C" size_t qcd_field_bytes(const qcd_ctx *ctx, int kind)
     case QCD_SPINOR_ODD: return half_spinor_bytes(ctx);
     case QCD_SPINOR_FULL: return 2 * half_spinor_bytes(ctx);
     case QCD_GAUGE: return (size_t)ctx->L.Vh * 72 * 2 * ctx->rsize;
+    case QCD_GAUGE_2ROW: return (size_t)ctx->L.Vh * 48 * 2 * ctx->rsize;
+    case QCD_COLOUR_MATRIX: return (size_t)ctx->L.Vh * 18 * 2 * ctx->rsize;
     default: return 0;
     }
 }
 
 extern "C" size_t qcd_workspace_bytes(const qcd_ctx *ctx) { return ctx ? 4 * half_spinor_bytes(ctx) : 0; }
+
+extern "C" size_t qcd_workspace_bytes_multi(const qcd_ctx *ctx, int n)
+{
+    return (ctx && n >= 1 && n <= MAXRHS) ? (size_t)n * 4 * half_spinor_bytes(ctx) : 0;
+}
 
 static int blas_n16(const qcd_ctx *c) { return (int)(half_spinor_bytes(c) / 16); }
 static int blas_grid(const qcd_ctx *c) { const int per = BLAS_BLOCK * BLAS_ITEMS; return (blas_n16(c) + per - 1) / per; }
@@ -159,13 +171,13 @@ extern "C" qcd_status qcd_init(qcd_ctx **out, const int dims[4], int precision, 
     c->d_scal = c->d_aux = nullptr; c->d_partials = nullptr; c->h_scal = nullptr; c->d_stage = nullptr;
     for (int i = 0; i < POLL_SLOTS; ++i) c->poll_ev[i] = nullptr;
 
-    c->partials_cap = dslash_grid_max(c) > blas_grid(c) ? dslash_grid_max(c) : blas_grid(c);
+    c->partials_cap = MAXRHS * (dslash_grid_max(c) > blas_grid(c) ? dslash_grid_max(c) : blas_grid(c));
     cudaError_t err = cudaSuccess;
-    if (err == cudaSuccess) err = cudaMalloc(&c->d_scal, 2 * sizeof(CgScalars));
-    if (err == cudaSuccess) err = cudaMemset(c->d_scal, 0, 2 * sizeof(CgScalars));
+    if (err == cudaSuccess) err = cudaMalloc(&c->d_scal, (MAXRHS + 1) * sizeof(CgScalars));
+    if (err == cudaSuccess) err = cudaMemset(c->d_scal, 0, (MAXRHS + 1) * sizeof(CgScalars));
     if (err == cudaSuccess) err = cudaMalloc(&c->d_partials, (size_t)c->partials_cap * sizeof(double));
     if (err == cudaSuccess) err = cudaMalloc(&c->d_stage, STAGE_BYTES);
-    if (err == cudaSuccess) err = cudaMallocHost(&c->h_scal, POLL_SLOTS * sizeof(CgScalars));
+    if (err == cudaSuccess) err = cudaMallocHost(&c->h_scal, POLL_SLOTS * MAXRHS * sizeof(CgScalars));
     for (int i = 0; i < POLL_SLOTS && err == cudaSuccess; ++i) err = cudaEventCreateWithFlags(&c->poll_ev[i], cudaEventDisableTiming);
     if (err == cudaSuccess) err = cudaEventCreate(&c->cg.ev_begin);
     if (err == cudaSuccess) err = cudaEventCreate(&c->cg.ev_end);
@@ -174,7 +186,7 @@ extern "C" qcd_status qcd_init(qcd_ctx **out, const int dims[4], int precision, 
         qcd_finalize(c);
         return err == cudaErrorMemoryAllocation ? QCD_ENOMEM : QCD_ECUDA;
     }
-    c->d_aux = c->d_scal + 1;
+    c->d_aux = c->d_scal + MAXRHS;
     *out = c;
     return QCD_OK;
 }
@@ -210,7 +222,7 @@ extern "C" qcd_status qcd_field_alloc(qcd_ctx *ctx, int kind, void *device_ptr, 
     if (nbytes < need) return fail(ctx, QCD_EINVAL, "qcd_field_alloc: buffer smaller than qcd_field_bytes");
     qcd_field *f = new (std::nothrow) qcd_field();
     if (!f) return fail(ctx, QCD_ENOMEM, "qcd_field_alloc: host allocation failed");
-    f->ctx = ctx; f->kind = kind; f->ptr = device_ptr; f->nbytes = nbytes;
+    f->ctx = ctx; f->kind = kind; f->ptr = device_ptr; f->nbytes = nbytes; f->tg = 0;
     *out = f;
     return QCD_OK;
 }
@@ -300,31 +312,38 @@ extern "C" qcd_status qcd_set_dslash_variant(qcd_ctx *ctx, int variant)
 // ------------------------------------------------------------------------------------------
 // upload / download
 // ------------------------------------------------------------------------------------------
+static bool is_gauge_kind(int kind) { return kind == QCD_GAUGE || kind == QCD_GAUGE_2ROW; }
+static bool is_spinor_kind(int kind) { return kind == QCD_SPINOR_EVEN || kind == QCD_SPINOR_ODD || kind == QCD_SPINOR_FULL; }
+static int gauge_nrow(const qcd_field *U) { return U->kind == QCD_GAUGE_2ROW ? 2 : 3; }
+
 template <typename T>
 static qcd_status transfer_t(qcd_ctx *c, const qcd_field *f, const void *host_in, void *host_out)
 {
     typedef typename Cplx<T>::type C;
     const bool up = host_in != nullptr;
-    const bool gauge = f->kind == QCD_GAUGE;
-    const size_t per_site = (gauge ? 36 : 3) * sizeof(C);
+    const bool matrix = !is_spinor_kind(f->kind);
+    const int nmu = f->kind == QCD_COLOUR_MATRIX ? 1 : 4;
+    const int nrow = f->kind == QCD_GAUGE_2ROW ? 2 : 3;
+    const unsigned per = matrix ? (unsigned)nmu * 9u : 3u;       // complex numbers per site in the host layout
+    const size_t per_site = per * sizeof(C);
     const unsigned V = 2u * (unsigned)c->L.Vh;
     unsigned chunk = (unsigned)(STAGE_BYTES / per_site);
     C *even = nullptr, *odd = nullptr;
-    if (!gauge) { even = (C *)half_ptr(f, 0); odd = (C *)half_ptr(f, 1); }
+    if (!matrix) { even = (C *)half_ptr(f, 0); odd = (C *)half_ptr(f, 1); }
     for (unsigned i0 = 0; i0 < V; i0 += chunk) {
         const unsigned n = (V - i0 < chunk) ? V - i0 : chunk;
-        const unsigned nthreads = n * (gauge ? 36u : 3u);
+        const unsigned nthreads = n * per;
         const unsigned grid = (nthreads + 255) / 256;
         if (up) {
             CU(c, cudaMemcpyAsync(c->d_stage, (const char *)host_in + (size_t)i0 * per_site, (size_t)n * per_site,
                                   cudaMemcpyHostToDevice, c->stream));
             LaunchScope ls(c, QCD_K_MISC);
-            if (gauge) gauge_scatter_kernel<C><<<grid, 256, 0, c->stream>>>(c->L, (const C *)c->d_stage, i0, n, (C *)f->ptr);
+            if (matrix) matrix_scatter_kernel<C><<<grid, 256, 0, c->stream>>>(c->L, (const C *)c->d_stage, i0, n, (C *)f->ptr, nmu, nrow);
             else spinor_scatter_kernel<C><<<grid, 256, 0, c->stream>>>(c->L, (const C *)c->d_stage, i0, n, even, odd);
         } else {
             {
                 LaunchScope ls(c, QCD_K_MISC);
-                if (gauge) gauge_gather_kernel<C><<<grid, 256, 0, c->stream>>>(c->L, (C *)c->d_stage, i0, n, (const C *)f->ptr);
+                if (matrix) matrix_gather_kernel<C><<<grid, 256, 0, c->stream>>>(c->L, (C *)c->d_stage, i0, n, (const C *)f->ptr, nmu, nrow);
                 else spinor_gather_kernel<C><<<grid, 256, 0, c->stream>>>(c->L, (C *)c->d_stage, i0, n, even, odd);
             }
             CU(c, cudaMemcpyAsync((char *)host_out + (size_t)i0 * per_site, c->d_stage, (size_t)n * per_site,
@@ -340,6 +359,7 @@ extern "C" qcd_status qcd_field_upload(qcd_field *f, const void *host)
 {
     if (!f) return QCD_EINVAL;
     if (!host) return fail(f->ctx, QCD_EINVAL, "qcd_field_upload: NULL host pointer");
+    f->tg = 0;
     return f->ctx->prec == 64 ? transfer_t<double>(f->ctx, f, host, nullptr) : transfer_t<float>(f->ctx, f, host, nullptr);
 }
 
@@ -353,89 +373,94 @@ extern "C" qcd_status qcd_field_download(const qcd_field *f, void *host)
 // ------------------------------------------------------------------------------------------
 // Dslash launches
 // ------------------------------------------------------------------------------------------
-template <typename T, int MODE, int BLOCK, int MINB>
-static void launch_dslash_cfg(qcd_ctx *c, const DslashArgs<T> &a)
+// out[r](parity) = D in[r](1-parity), r < n; mode >= 1 adds the M epilogue with v[r] (parity of out)
+static qcd_status dslash_launch(qcd_ctx *c, int mode, const qcd_field *U, int n, void *const *out, const void *const *in,
+                                int parity, const void *const *v, double m, CgScalars *scal, int check_flag)
 {
-    const int grid = (c->L.Vh + BLOCK - 1) / BLOCK;
-    dslash_kernel<T, MODE, BLOCK, MINB><<<grid, BLOCK, 0, c->stream>>>(a);
-}
-
-template <typename T, int MODE>
-static void launch_dslash(qcd_ctx *c, const DslashArgs<T> &a)
-{
-    LaunchScope ls(c, MODE == 0 ? QCD_K_DSLASH : QCD_K_DSLASH_EPI);
-    switch (c->variant) {
-    default:
-    case 0: launch_dslash_cfg<T, MODE, 128, 4>(c, a); break;
-    case 1: launch_dslash_cfg<T, MODE, 64, 8>(c, a); break;
-    case 2: launch_dslash_cfg<T, MODE, 256, 2>(c, a); break;
-    case 3: launch_dslash_cfg<T, MODE, 128, 3>(c, a); break;
+    DslashLaunch d;
+    d.mode = mode; d.tg = U->tg; d.nrhs = n; d.variant = c->variant;
+    d.L = c->L; d.parity = parity; d.U = U->ptr;
+    for (int r = 0; r < MAXRHS; ++r) {
+        d.in[r] = r < n ? in[r] : nullptr;
+        d.out[r] = r < n ? out[r] : nullptr;
+        d.v[r] = (r < n && v) ? v[r] : nullptr;
     }
-}
-
-// out(parity) = D in(1-parity); MODE >= 1 adds the M epilogue with v (same parity as out)
-template <typename T, int MODE>
-static qcd_status dslash_t(qcd_ctx *c, const void *U, void *out, const void *in, int parity, const void *v, double m,
-                           CgScalars *scal, int check_flag)
-{
-    typedef typename Cplx<T>::type C;
-    DslashArgs<T> a;
-    a.L = c->L; a.parity = parity;
-    a.U = (const C *)U; a.in = (const C *)in; a.out = (C *)out; a.v = (const C *)v;
-    a.m2 = (T)(m * m);
-    a.partials = c->d_partials; a.scal = scal; a.check_flag = check_flag;
-    launch_dslash<T, MODE>(c, a);
-    CU(c, cudaGetLastError());
+    d.m2 = m * m; d.partials = c->d_partials; d.scal = scal; d.check_flag = check_flag; d.stream = c->stream;
+    LaunchScope ls(c, mode == 0 ? QCD_K_DSLASH : QCD_K_DSLASH_EPI);
+    cudaError_t e;
+    if (c->prec == 64) e = gauge_nrow(U) == 3 ? launch_dslash_f64_r3(d) : launch_dslash_f64_r2(d);
+    else e = gauge_nrow(U) == 3 ? launch_dslash_f32_r3(d) : launch_dslash_f32_r2(d);
+    if (e != cudaSuccess) return fail(c, QCD_ECUDA, "dslash launch: %s", cudaGetErrorString(e));
     return QCD_OK;
 }
 
-static qcd_status dslash_dispatch(qcd_ctx *c, int mode, const void *U, void *out, const void *in, int parity,
-                                  const void *v, double m, CgScalars *scal, int check_flag)
+static qcd_status dslash_one(qcd_ctx *c, int mode, const qcd_field *U, void *out, const void *in, int parity,
+                             const void *v, double m, CgScalars *scal, int check_flag)
 {
-    if (c->prec == 64) {
-        if (mode == 0) return dslash_t<double, 0>(c, U, out, in, parity, v, m, scal, check_flag);
-        if (mode == 1) return dslash_t<double, 1>(c, U, out, in, parity, v, m, scal, check_flag);
-        return dslash_t<double, 2>(c, U, out, in, parity, v, m, scal, check_flag);
-    }
-    if (mode == 0) return dslash_t<float, 0>(c, U, out, in, parity, v, m, scal, check_flag);
-    if (mode == 1) return dslash_t<float, 1>(c, U, out, in, parity, v, m, scal, check_flag);
-    return dslash_t<float, 2>(c, U, out, in, parity, v, m, scal, check_flag);
+    return dslash_launch(c, mode, U, 1, &out, &in, parity, v ? &v : nullptr, m, scal, check_flag);
 }
 
 static qcd_status check_gauge(qcd_ctx *ctx, const qcd_field *U, const char *who)
 {
-    if (!U || U->ctx != ctx || U->kind != QCD_GAUGE) return fail(ctx, QCD_EINVAL, "%s: U must be a QCD_GAUGE field of this context", who);
+    if (!U || U->ctx != ctx || !is_gauge_kind(U->kind))
+        return fail(ctx, QCD_EINVAL, "%s: U must be a QCD_GAUGE or QCD_GAUGE_2ROW field of this context", who);
     return QCD_OK;
 }
 
-static qcd_status dslash_public(qcd_ctx *ctx, const qcd_field *U, qcd_field *out, const qcd_field *in, int out_parity, const char *who)
+static qcd_status dslash_public(qcd_ctx *ctx, const qcd_field *U, int n, qcd_field *const *out, const qcd_field *const *in,
+                                int out_parity, const char *who)
 {
     if (!ctx) return QCD_EINVAL;
     qcd_status s = check_gauge(ctx, U, who);
     if (s) return s;
-    if (!out || !in || out->ctx != ctx || in->ctx != ctx) return fail(ctx, QCD_EINVAL, "%s: fields must belong to this context", who);
-    void *o = half_ptr(out, out_parity);
-    const void *i = half_ptr(in, 1 - out_parity);
-    if (!o || !i) return fail(ctx, QCD_EINVAL, "%s: spinor parity / kind mismatch", who);
-    if (o == i || out->ptr == in->ptr) return fail(ctx, QCD_EINVAL, "%s: out must not alias in", who);
-    return dslash_dispatch(ctx, 0, U->ptr, o, i, out_parity, nullptr, 0.0, ctx->d_aux, 0);
+    if (n < 1 || n > MAXRHS) return fail(ctx, QCD_EINVAL, "%s: n must be 1 .. QCD_MAX_RHS", who);
+    if (!out || !in) return fail(ctx, QCD_EINVAL, "%s: NULL field array", who);
+    void *o[MAXRHS]; const void *i[MAXRHS];
+    for (int r = 0; r < n; ++r) {
+        if (!out[r] || !in[r] || out[r]->ctx != ctx || in[r]->ctx != ctx) return fail(ctx, QCD_EINVAL, "%s: fields must belong to this context", who);
+        o[r] = half_ptr(out[r], out_parity);
+        i[r] = half_ptr(in[r], 1 - out_parity);
+        if (!o[r] || !i[r]) return fail(ctx, QCD_EINVAL, "%s: spinor parity / kind mismatch", who);
+        if (out[r]->ptr == in[r]->ptr) return fail(ctx, QCD_EINVAL, "%s: out must not alias in", who);
+        for (int q = 0; q < r; ++q) if (o[q] == o[r]) return fail(ctx, QCD_EINVAL, "%s: two outputs alias", who);
+    }
+    return dslash_launch(ctx, 0, U, n, o, i, out_parity, nullptr, 0.0, ctx->d_aux, 0);
 }
 
 extern "C" qcd_status qcd_dslash_eo(qcd_ctx *ctx, const qcd_field *U, qcd_field *out_even, const qcd_field *in_odd)
 {
-    return dslash_public(ctx, U, out_even, in_odd, 0, "qcd_dslash_eo");
+    return dslash_public(ctx, U, 1, &out_even, &in_odd, 0, "qcd_dslash_eo");
 }
 
 extern "C" qcd_status qcd_dslash_oe(qcd_ctx *ctx, const qcd_field *U, qcd_field *out_odd, const qcd_field *in_even)
 {
-    return dslash_public(ctx, U, out_odd, in_even, 1, "qcd_dslash_oe");
+    return dslash_public(ctx, U, 1, &out_odd, &in_even, 1, "qcd_dslash_oe");
 }
 
-// workspace carving: r, p, Ap (even half-fields) then t (odd half-field)
-static void *ws_r(qcd_ctx *c) { return c->ws; }
-static void *ws_p(qcd_ctx *c) { return (char *)c->ws + half_spinor_bytes(c); }
-static void *ws_Ap(qcd_ctx *c) { return (char *)c->ws + 2 * half_spinor_bytes(c); }
-static void *ws_t(qcd_ctx *c) { return (char *)c->ws + 3 * half_spinor_bytes(c); }
+extern "C" qcd_status qcd_dslash_eo_multi(qcd_ctx *ctx, const qcd_field *U, int n, qcd_field *const *out_even, const qcd_field *const *in_odd)
+{
+    return dslash_public(ctx, U, n, out_even, in_odd, 0, "qcd_dslash_eo_multi");
+}
+
+extern "C" qcd_status qcd_dslash_oe_multi(qcd_ctx *ctx, const qcd_field *U, int n, qcd_field *const *out_odd, const qcd_field *const *in_even)
+{
+    return dslash_public(ctx, U, n, out_odd, in_even, 1, "qcd_dslash_oe_multi");
+}
+
+// workspace carving for n right-hand sides: r[n], p[n], Ap[n] (even half-fields) then t[n] (odd)
+static void *ws_at(qcd_ctx *c, int block, int n, int rhs) { return (char *)c->ws + ((size_t)block * n + rhs) * half_spinor_bytes(c); }
+static void *ws_r(qcd_ctx *c, int n = 1, int rhs = 0) { return ws_at(c, 0, n, rhs); }
+static void *ws_p(qcd_ctx *c, int n = 1, int rhs = 0) { return ws_at(c, 1, n, rhs); }
+static void *ws_Ap(qcd_ctx *c, int n = 1, int rhs = 0) { return ws_at(c, 2, n, rhs); }
+static void *ws_t(qcd_ctx *c, int n = 1, int rhs = 0) { return ws_at(c, 3, n, rhs); }
+
+// out = m^2 in - D_eo D_oe in on raw even half-field pointers (workspace t is the intermediate)
+static qcd_status apply_M_raw(qcd_ctx *ctx, const qcd_field *U, void *out, const void *in, double m)
+{
+    qcd_status s = dslash_one(ctx, 0, U, ws_t(ctx), in, 1, nullptr, 0.0, ctx->d_aux, 0);      // t = D_oe in
+    if (s) return s;
+    return dslash_one(ctx, 1, U, out, ws_t(ctx), 0, in, m, ctx->d_aux, 0);                    // out = m^2 in - D_eo t
+}
 
 extern "C" qcd_status qcd_apply_M(qcd_ctx *ctx, const qcd_field *U, qcd_field *out_even, const qcd_field *in_even, double m)
 {
@@ -450,9 +475,7 @@ extern "C" qcd_status qcd_apply_M(qcd_ctx *ctx, const qcd_field *U, qcd_field *o
     const void *i = half_ptr(in_even, 0);
     if (!o || !i) return fail(ctx, QCD_EINVAL, "qcd_apply_M: both spinors must hold even sites");
     if (o == i) return fail(ctx, QCD_EINVAL, "qcd_apply_M: out must not alias in");
-    s = dslash_dispatch(ctx, 0, U->ptr, ws_t(ctx), i, 1, nullptr, 0.0, ctx->d_aux, 0);      // t = D_oe in
-    if (s) return s;
-    return dslash_dispatch(ctx, 1, U->ptr, o, ws_t(ctx), 0, i, m, ctx->d_aux, 0);           // out = m^2 in - D_eo t
+    return apply_M_raw(ctx, U, o, i, m);
 }
 
 // ------------------------------------------------------------------------------------------
@@ -479,15 +502,28 @@ extern "C" qcd_status qcd_re_dot(qcd_ctx *ctx, const qcd_field *a, const qcd_fie
 }
 
 // ------------------------------------------------------------------------------------------
-// CG
+// CG (n right-hand sides in lock step; qcd_cg_solve is n = 1)
 // ------------------------------------------------------------------------------------------
+template <typename T>
+static RhsPtrs<typename Vec16<T>::type> rhs_ptrs(const qcd_ctx *c)
+{
+    typedef typename Vec16<T>::type V;
+    RhsPtrs<V> p;
+    for (int r = 0; r < MAXRHS; ++r) {
+        p.x[r] = r < c->cg.n ? (V *)c->cg.x[r] : nullptr;
+        p.b[r] = r < c->cg.n ? (const V *)c->cg.b[r] : nullptr;
+    }
+    return p;
+}
+
 template <typename T>
 static qcd_status cg_begin_t(qcd_ctx *c)
 {
     typedef typename Vec16<T>::type V;
+    const int n = c->cg.n;
     LaunchScope ls(c, QCD_K_MISC);
-    cg_init_kernel<T><<<blas_grid(c), BLAS_BLOCK, 0, c->stream>>>(
-        blas_n16(c), (const V *)c->cg.b->ptr, (V *)c->cg.x->ptr, (V *)ws_r(c), (V *)ws_p(c),
+    cg_init_kernel<T><<<dim3(blas_grid(c), n), BLAS_BLOCK, 0, c->stream>>>(
+        blas_n16(c), rhs_ptrs<T>(c), (V *)ws_r(c, n), (V *)ws_p(c, n),
         c->cg.tol, c->cg.maxiter, c->d_partials, c->d_scal);
     CU(c, cudaGetLastError());
     return QCD_OK;
@@ -499,43 +535,60 @@ template <typename T>
 static qcd_status cg_iteration_t(qcd_ctx *c)
 {
     typedef typename Vec16<T>::type V;
-    qcd_status s = dslash_t<T, 0>(c, c->cg.U->ptr, ws_t(c), ws_p(c), 1, nullptr, 0.0, c->d_scal, 1);
+    const int n = c->cg.n;
+    void *t[MAXRHS], *Ap[MAXRHS];
+    const void *p[MAXRHS], *tc[MAXRHS];
+    for (int r = 0; r < n; ++r) { t[r] = ws_t(c, n, r); Ap[r] = ws_Ap(c, n, r); p[r] = ws_p(c, n, r); tc[r] = t[r]; }
+    qcd_status s = dslash_launch(c, 0, c->cg.U, n, t, p, 1, nullptr, 0.0, c->d_scal, 1);
     if (s) return s;
-    s = dslash_t<T, 2>(c, c->cg.U->ptr, ws_Ap(c), ws_t(c), 0, ws_p(c), c->cg.m, c->d_scal, 1);
+    s = dslash_launch(c, 2, c->cg.U, n, Ap, tc, 0, p, c->cg.m, c->d_scal, 1);
     if (s) return s;
     {
         LaunchScope ls(c, QCD_K_UPDATE_XR);
-        cg_update_xr_kernel<T><<<blas_grid(c), BLAS_BLOCK, 0, c->stream>>>(
-            blas_n16(c), (V *)c->cg.x->ptr, (V *)ws_r(c), (const V *)ws_p(c), (const V *)ws_Ap(c), c->d_partials, c->d_scal);
+        cg_update_xr_kernel<T><<<dim3(blas_grid(c), n), BLAS_BLOCK, 0, c->stream>>>(
+            blas_n16(c), rhs_ptrs<T>(c), (V *)ws_r(c, n), (const V *)ws_p(c, n), (const V *)ws_Ap(c, n), c->d_partials, c->d_scal);
     }
     {
         LaunchScope ls(c, QCD_K_UPDATE_P);
-        cg_update_p_kernel<T><<<blas_grid(c), BLAS_BLOCK, 0, c->stream>>>(blas_n16(c), (V *)ws_p(c), (const V *)ws_r(c), c->d_scal);
+        cg_update_p_kernel<T><<<dim3(blas_grid(c), n), BLAS_BLOCK, 0, c->stream>>>(blas_n16(c), (V *)ws_p(c, n), (const V *)ws_r(c, n), c->d_scal);
     }
     CU(c, cudaGetLastError());
+    return QCD_OK;
+}
+
+extern "C" qcd_status qcd_cg_begin_multi(qcd_ctx *ctx, const qcd_field *U, int n, const qcd_field *const *b, qcd_field *const *x,
+                                         double m, double tol, int maxiter)
+{
+    if (!ctx) return QCD_EINVAL;
+    qcd_status s = check_gauge(ctx, U, "qcd_cg_begin");
+    if (s) return s;
+    if (n < 1 || n > MAXRHS) return fail(ctx, QCD_EINVAL, "qcd_cg: n must be 1 .. QCD_MAX_RHS");
+    if (!(m >= 0.0)) return fail(ctx, QCD_EINVAL, "qcd_cg: m must be >= 0");
+    if (!(tol > 0.0)) return fail(ctx, QCD_EINVAL, "qcd_cg: tol must be > 0");
+    if (maxiter < 0) return fail(ctx, QCD_EINVAL, "qcd_cg: maxiter must be >= 0");
+    if (!b || !x) return fail(ctx, QCD_EINVAL, "qcd_cg: NULL field array");
+    for (int r = 0; r < n; ++r) {
+        if (!b[r] || !x[r] || b[r]->ctx != ctx || x[r]->ctx != ctx || b[r]->kind != QCD_SPINOR_EVEN || x[r]->kind != QCD_SPINOR_EVEN)
+            return fail(ctx, QCD_EINVAL, "qcd_cg: b and x must be QCD_SPINOR_EVEN fields of this context");
+        if (b[r]->ptr == x[r]->ptr) return fail(ctx, QCD_EINVAL, "qcd_cg: x must not alias b");
+        for (int q = 0; q < r; ++q) if (x[q]->ptr == x[r]->ptr) return fail(ctx, QCD_EINVAL, "qcd_cg: two solutions alias");
+    }
+    if (!ctx->ws || ctx->ws_bytes < qcd_workspace_bytes_multi(ctx, n))
+        return fail(ctx, QCD_EINVAL, "qcd_cg: workspace missing or smaller than qcd_workspace_bytes_multi (qcd_set_workspace)");
+    if (ctx->cg.active) return fail(ctx, QCD_EINVAL, "qcd_cg_begin: a solve is already in progress");
+    ctx->cg.U = U; ctx->cg.n = n; ctx->cg.m = m; ctx->cg.tol = tol; ctx->cg.maxiter = maxiter;
+    for (int r = 0; r < n; ++r) { ctx->cg.b[r] = b[r]->ptr; ctx->cg.x[r] = x[r]->ptr; }
+    CU(ctx, cudaEventRecord(ctx->cg.ev_begin, ctx->stream));
+    s = ctx->prec == 64 ? cg_begin_t<double>(ctx) : cg_begin_t<float>(ctx);
+    if (s) return s;
+    ctx->cg.active = true;
     return QCD_OK;
 }
 
 extern "C" qcd_status qcd_cg_begin(qcd_ctx *ctx, const qcd_field *U, const qcd_field *b, qcd_field *x,
                                    double m, double tol, int maxiter)
 {
-    if (!ctx) return QCD_EINVAL;
-    qcd_status s = check_gauge(ctx, U, "qcd_cg_begin");
-    if (s) return s;
-    if (!(m >= 0.0)) return fail(ctx, QCD_EINVAL, "qcd_cg: m must be >= 0");
-    if (!(tol > 0.0)) return fail(ctx, QCD_EINVAL, "qcd_cg: tol must be > 0");
-    if (maxiter < 0) return fail(ctx, QCD_EINVAL, "qcd_cg: maxiter must be >= 0");
-    if (!b || !x || b->ctx != ctx || x->ctx != ctx || b->kind != QCD_SPINOR_EVEN || x->kind != QCD_SPINOR_EVEN)
-        return fail(ctx, QCD_EINVAL, "qcd_cg: b and x must be QCD_SPINOR_EVEN fields of this context");
-    if (b->ptr == x->ptr) return fail(ctx, QCD_EINVAL, "qcd_cg: x must not alias b");
-    if (!ctx->ws) return fail(ctx, QCD_EINVAL, "qcd_cg: no workspace bound (qcd_set_workspace)");
-    if (ctx->cg.active) return fail(ctx, QCD_EINVAL, "qcd_cg_begin: a solve is already in progress");
-    ctx->cg.U = U; ctx->cg.b = b; ctx->cg.x = x; ctx->cg.m = m; ctx->cg.tol = tol; ctx->cg.maxiter = maxiter;
-    CU(ctx, cudaEventRecord(ctx->cg.ev_begin, ctx->stream));
-    s = ctx->prec == 64 ? cg_begin_t<double>(ctx) : cg_begin_t<float>(ctx);
-    if (s) return s;
-    ctx->cg.active = true;
-    return QCD_OK;
+    return qcd_cg_begin_multi(ctx, U, 1, &b, &x, m, tol, maxiter);
 }
 
 extern "C" qcd_status qcd_cg_iterate(qcd_ctx *ctx, int n)
@@ -550,47 +603,71 @@ extern "C" qcd_status qcd_cg_iterate(qcd_ctx *ctx, int n)
     return QCD_OK;
 }
 
-static qcd_status read_scalars(qcd_ctx *ctx, CgScalars *out)
+// copies the cg.n recurrence states to pinned slot 0 and returns a pointer to them
+static qcd_status read_scalars(qcd_ctx *ctx, const CgScalars **out)
 {
-    CU(ctx, cudaMemcpyAsync(&ctx->h_scal[0], ctx->d_scal, sizeof(CgScalars), cudaMemcpyDeviceToHost, ctx->stream));
+    CU(ctx, cudaMemcpyAsync(&ctx->h_scal[0], ctx->d_scal, ctx->cg.n * sizeof(CgScalars), cudaMemcpyDeviceToHost, ctx->stream));
     CU(ctx, cudaStreamSynchronize(ctx->stream));
-    *out = ctx->h_scal[0];
+    *out = &ctx->h_scal[0];
     return QCD_OK;
 }
 
 static double rel_resid_of(const CgScalars &s) { return s.bb > 0.0 ? sqrt(s.rr / s.bb) : 0.0; }
 
+// state of a lock-step solve: running while any right-hand side runs, else the worst outcome
+static int joint_state(const CgScalars *s, int n)
+{
+    int st = 1;
+    for (int r = 0; r < n; ++r) {
+        if (s[r].flag == 0) return 0;
+        if (s[r].flag > st) st = s[r].flag;
+    }
+    return st;
+}
+
 extern "C" qcd_status qcd_cg_poll(qcd_ctx *ctx, int *state, int *iters, double *rel_resid)
 {
     if (!ctx) return QCD_EINVAL;
     if (!ctx->cg.active) return fail(ctx, QCD_EINVAL, "qcd_cg_poll: no solve in progress");
-    CgScalars s;
+    const CgScalars *s;
     qcd_status st = read_scalars(ctx, &s);
     if (st) return st;
-    if (state) *state = s.flag;
-    if (iters) *iters = s.k;
-    if (rel_resid) *rel_resid = rel_resid_of(s);
+    int k = 0; double rel = 0.0;
+    for (int r = 0; r < ctx->cg.n; ++r) { if (s[r].k > k) k = s[r].k; if (rel_resid_of(s[r]) > rel) rel = rel_resid_of(s[r]); }
+    if (state) *state = joint_state(s, ctx->cg.n);
+    if (iters) *iters = k;
+    if (rel_resid) *rel_resid = rel;
     return QCD_OK;
 }
 
-extern "C" qcd_status qcd_cg_finish(qcd_ctx *ctx, qcd_cg_info *info)
+extern "C" qcd_status qcd_cg_finish_multi(qcd_ctx *ctx, qcd_cg_info *info)
 {
     if (!ctx) return QCD_EINVAL;
     if (!ctx->cg.active) return fail(ctx, QCD_EINVAL, "qcd_cg_finish: no solve in progress");
     ctx->cg.active = false;
     CU(ctx, cudaEventRecord(ctx->cg.ev_end, ctx->stream));
-    CgScalars s;
+    const CgScalars *s;
     qcd_status st = read_scalars(ctx, &s);
     if (st) return st;
     float ms = 0.f;
     CU(ctx, cudaEventElapsedTime(&ms, ctx->cg.ev_begin, ctx->cg.ev_end));
-    if (info) {
-        info->iters = s.k; info->converged = s.flag == 1; info->rel_resid = rel_resid_of(s);
-        info->bnorm2 = s.bb; info->seconds = ms * 1e-3;
+    qcd_status res = QCD_OK;
+    for (int r = 0; r < ctx->cg.n; ++r) {
+        if (info) {
+            info[r].iters = s[r].k; info[r].converged = s[r].flag == 1; info[r].rel_resid = rel_resid_of(s[r]);
+            info[r].bnorm2 = s[r].bb; info[r].seconds = ms * 1e-3;
+        }
+        if (res == QCD_OK && s[r].flag != 1) res = s[r].flag == 3 ? QCD_EBREAKDOWN : QCD_ENOTCONVERGED;
     }
-    if (s.flag == 1) return QCD_OK;
-    if (s.flag == 3) return fail(ctx, QCD_EBREAKDOWN, "qcd_cg: breakdown (<p,Mp> <= 0 or NaN)");
-    return fail(ctx, QCD_ENOTCONVERGED, "qcd_cg: not converged");
+    if (res == QCD_EBREAKDOWN) return fail(ctx, res, "qcd_cg: breakdown (<p,Mp> <= 0 or NaN)");
+    if (res == QCD_ENOTCONVERGED) return fail(ctx, res, "qcd_cg: not converged");
+    return QCD_OK;
+}
+
+extern "C" qcd_status qcd_cg_finish(qcd_ctx *ctx, qcd_cg_info *info)
+{
+    if (ctx && ctx->cg.active && ctx->cg.n != 1) return fail(ctx, QCD_EINVAL, "qcd_cg_finish: a multi solve is in progress (qcd_cg_finish_multi)");
+    return qcd_cg_finish_multi(ctx, info);
 }
 
 // Host loop: keep two chunks of iterations in flight; after each chunk the scalars are copied
@@ -599,37 +676,43 @@ extern "C" qcd_status qcd_cg_finish(qcd_ctx *ctx, qcd_cg_info *info)
 // stop flag was set exit at their first instruction, so x is frozen at the exact iteration.
 static qcd_status cg_run(qcd_ctx *ctx)
 {
-    const int maxiter = ctx->cg.maxiter;
+    const int maxiter = ctx->cg.maxiter, n = ctx->cg.n;
     int enq = 0, head = 0, tail = 0, pending = 0, chunk = 8;
     bool first = true;
     for (;;) {
         while (pending < POLL_SLOTS && (enq < maxiter || first)) {
-            const int n = maxiter - enq < chunk ? maxiter - enq : chunk;
-            qcd_status s = qcd_cg_iterate(ctx, n);
+            const int it = maxiter - enq < chunk ? maxiter - enq : chunk;
+            qcd_status s = qcd_cg_iterate(ctx, it);
             if (s) return s;
-            enq += n;
-            CU(ctx, cudaMemcpyAsync(&ctx->h_scal[head], ctx->d_scal, sizeof(CgScalars), cudaMemcpyDeviceToHost, ctx->stream));
+            enq += it;
+            CU(ctx, cudaMemcpyAsync(&ctx->h_scal[head * MAXRHS], ctx->d_scal, n * sizeof(CgScalars), cudaMemcpyDeviceToHost, ctx->stream));
             CU(ctx, cudaEventRecord(ctx->poll_ev[head], ctx->stream));
             head = (head + 1) % POLL_SLOTS; ++pending; first = false;
             if (chunk < 64) chunk *= 2;
         }
         CU(ctx, cudaEventSynchronize(ctx->poll_ev[tail]));
-        const int flag = ctx->h_scal[tail].flag;
+        const int state = joint_state(&ctx->h_scal[tail * MAXRHS], n);
         tail = (tail + 1) % POLL_SLOTS; --pending;
-        if (flag != 0) break;
+        if (state != 0) break;
         if (pending == 0 && enq >= maxiter) break;   // defensive: flag 2 is set when k reaches maxiter
     }
     return QCD_OK;
 }
 
-extern "C" qcd_status qcd_cg_solve(qcd_ctx *ctx, const qcd_field *U, const qcd_field *b, qcd_field *x,
-                                   double m, double tol, int maxiter, qcd_cg_info *info)
+extern "C" qcd_status qcd_cg_solve_multi(qcd_ctx *ctx, const qcd_field *U, int n, const qcd_field *const *b, qcd_field *const *x,
+                                         double m, double tol, int maxiter, qcd_cg_info *info)
 {
-    qcd_status s = qcd_cg_begin(ctx, U, b, x, m, tol, maxiter);
+    qcd_status s = qcd_cg_begin_multi(ctx, U, n, b, x, m, tol, maxiter);
     if (s) return s;
     s = cg_run(ctx);
     if (s) { ctx->cg.active = false; return s; }
-    return qcd_cg_finish(ctx, info);
+    return qcd_cg_finish_multi(ctx, info);
+}
+
+extern "C" qcd_status qcd_cg_solve(qcd_ctx *ctx, const qcd_field *U, const qcd_field *b, qcd_field *x,
+                                   double m, double tol, int maxiter, qcd_cg_info *info)
+{
+    return qcd_cg_solve_multi(ctx, U, 1, &b, &x, m, tol, maxiter, info);
 }
 
 extern "C" qcd_status qcd_cg_solve_host(qcd_ctx *ctx, const qcd_field *U, qcd_field *b_dev, qcd_field *x_dev,
@@ -656,4 +739,189 @@ extern "C" qcd_status qcd_cg_solve_host(qcd_ctx *ctx, const qcd_field *U, qcd_fi
     cudaEventDestroy(e0); cudaEventDestroy(e1);
     if (info) info->seconds = ms * 1e-3;
     return s ? s : solve;
+}
+
+// ------------------------------------------------------------------------------------------
+// Variants: two-row links, temporal gauge, precision conversion
+// ------------------------------------------------------------------------------------------
+extern "C" qcd_status qcd_gauge_compress(qcd_ctx *ctx, const qcd_field *U, qcd_field *U12)
+{
+    if (!ctx) return QCD_EINVAL;
+    if (!U || !U12 || U->ctx != ctx || U12->ctx != ctx || U->kind != QCD_GAUGE || U12->kind != QCD_GAUGE_2ROW)
+        return fail(ctx, QCD_EINVAL, "qcd_gauge_compress: need a QCD_GAUGE source and a QCD_GAUGE_2ROW destination of this context");
+    const size_t plane = (size_t)ctx->L.Vh * 2 * ctx->rsize;
+    // rows 0 and 1 of link (parity, mu) are its first 6 planes: 8 contiguous 6-plane copies
+    for (int pm = 0; pm < 8; ++pm)
+        CU(ctx, cudaMemcpyAsync((char *)U12->ptr + (size_t)pm * 6 * plane, (const char *)U->ptr + (size_t)pm * 9 * plane,
+                                6 * plane, cudaMemcpyDeviceToDevice, ctx->stream));
+    U12->tg = U->tg;
+    return QCD_OK;
+}
+
+extern "C" qcd_status qcd_gauge_set_temporal_unit(qcd_field *U, int on)
+{
+    if (!U) return QCD_EINVAL;
+    if (!is_gauge_kind(U->kind)) return fail(U->ctx, QCD_EINVAL, "qcd_gauge_set_temporal_unit: not a gauge field");
+    U->tg = on != 0;
+    return QCD_OK;
+}
+
+template <typename T>
+static void gauge_fix_t(qcd_ctx *c, const qcd_field *U, qcd_field *Uf, qcd_field *g)
+{
+    typedef typename Cplx<T>::type C;
+    const int vs = c->L.N0 * c->L.N1 * c->L.N2;
+    {
+        LaunchScope ls(c, QCD_K_MISC);
+        temporal_gauge_g_kernel<C><<<(vs + 127) / 128, 128, 0, c->stream>>>(c->L, (const C *)U->ptr, (C *)g->ptr);
+    }
+    for (int par = 0; par < 2; ++par) {
+        LaunchScope ls(c, QCD_K_MISC);
+        gauge_transform_kernel<C><<<(c->L.Vh + 127) / 128, 128, 0, c->stream>>>(c->L, par, (const C *)U->ptr, (const C *)g->ptr, (C *)Uf->ptr, 1);
+    }
+}
+
+extern "C" qcd_status qcd_gauge_fix_temporal(qcd_ctx *ctx, const qcd_field *U, qcd_field *U_fixed, qcd_field *g)
+{
+    if (!ctx) return QCD_EINVAL;
+    if (!U || !U_fixed || !g || U->ctx != ctx || U_fixed->ctx != ctx || g->ctx != ctx ||
+        U->kind != QCD_GAUGE || U_fixed->kind != QCD_GAUGE || g->kind != QCD_COLOUR_MATRIX)
+        return fail(ctx, QCD_EINVAL, "qcd_gauge_fix_temporal: need QCD_GAUGE U, QCD_GAUGE U_fixed and QCD_COLOUR_MATRIX g of this context");
+    if (U->ptr == U_fixed->ptr) return fail(ctx, QCD_EINVAL, "qcd_gauge_fix_temporal: U_fixed must not alias U");
+    if (ctx->prec == 64) gauge_fix_t<double>(ctx, U, U_fixed, g); else gauge_fix_t<float>(ctx, U, U_fixed, g);
+    CU(ctx, cudaGetLastError());
+    U_fixed->tg = 1;
+    return QCD_OK;
+}
+
+extern "C" qcd_status qcd_spinor_rotate(qcd_ctx *ctx, const qcd_field *g, qcd_field *out, const qcd_field *in, int dagger)
+{
+    if (!ctx) return QCD_EINVAL;
+    if (!g || !out || !in || g->ctx != ctx || out->ctx != ctx || in->ctx != ctx || g->kind != QCD_COLOUR_MATRIX ||
+        !is_spinor_kind(in->kind) || out->kind != in->kind)
+        return fail(ctx, QCD_EINVAL, "qcd_spinor_rotate: need a QCD_COLOUR_MATRIX g and two spinor fields of the same kind");
+    const int grid = (ctx->L.Vh + 127) / 128;
+    for (int par = 0; par < 2; ++par) {
+        void *o = half_ptr(out, par);
+        const void *i = half_ptr(in, par);
+        if (!o || !i) continue;
+        LaunchScope ls(ctx, QCD_K_MISC);
+        if (ctx->prec == 64)
+            spinor_rotate_kernel<double2><<<grid, 128, 0, ctx->stream>>>(ctx->L, par, (const double2 *)g->ptr, (const double2 *)i, (double2 *)o, dagger != 0);
+        else
+            spinor_rotate_kernel<float2><<<grid, 128, 0, ctx->stream>>>(ctx->L, par, (const float2 *)g->ptr, (const float2 *)i, (float2 *)o, dagger != 0);
+    }
+    CU(ctx, cudaGetLastError());
+    return QCD_OK;
+}
+
+extern "C" qcd_status qcd_field_convert(qcd_field *dst, const qcd_field *src)
+{
+    if (!dst || !src) return QCD_EINVAL;
+    qcd_ctx *cd = dst->ctx, *cs = src->ctx;
+    if (dst->kind != src->kind || cd->prec == cs->prec || memcmp(&cd->L, &cs->L, sizeof(Lattice)) != 0 || cd->stream != cs->stream)
+        return fail(cd, QCD_EINVAL, "qcd_field_convert: need the same kind and lattice, different precisions, one stream");
+    const size_t n = qcd_field_bytes(cs, src->kind) / cs->rsize;
+    const int grid = (int)((n + 255) / 256 < 148 * 16 ? (n + 255) / 256 : 148 * 16);
+    {
+        LaunchScope ls(cd, QCD_K_MISC);
+        if (cs->prec == 64) convert_kernel<double, float><<<grid, 256, 0, cd->stream>>>(n, (const double *)src->ptr, (float *)dst->ptr);
+        else convert_kernel<float, double><<<grid, 256, 0, cd->stream>>>(n, (const float *)src->ptr, (double *)dst->ptr);
+    }
+    CU(cd, cudaGetLastError());
+    dst->tg = src->tg;
+    return QCD_OK;
+}
+
+// ------------------------------------------------------------------------------------------
+// Mixed-precision defect-correction CG (reading R21)
+// ------------------------------------------------------------------------------------------
+// r = b - Mx (Mx may be NULL: r = b), <r,r> -> host
+static qcd_status mixed_residual(qcd_ctx *c, const void *b, const void *Mx, void *r, double *rr)
+{
+    {
+        LaunchScope ls(c, QCD_K_MISC);
+        mixed_residual_kernel<<<blas_grid(c), BLAS_BLOCK, 0, c->stream>>>(blas_n16(c), (const double2 *)b, (const double2 *)Mx, (double2 *)r, c->d_partials, c->d_aux);
+    }
+    CU(c, cudaGetLastError());
+    CU(c, cudaMemcpyAsync(&c->h_scal[0], c->d_aux, sizeof(CgScalars), cudaMemcpyDeviceToHost, c->stream));
+    CU(c, cudaStreamSynchronize(c->stream));
+    *rr = c->h_scal[0].dot;
+    return QCD_OK;
+}
+
+extern "C" qcd_status qcd_cg_solve_mixed(qcd_ctx *c64, qcd_ctx *c32, const qcd_field *U64, const qcd_field *U32,
+                                         const qcd_field *b, qcd_field *x, qcd_field *rhs32, qcd_field *e32,
+                                         double m, double tol, double inner_tol, int maxiter, int max_outer,
+                                         qcd_mixed_info *info)
+{
+    if (!c64) return QCD_EINVAL;
+    if (!c32 || c64->prec != 64 || c32->prec != 32 || memcmp(&c64->L, &c32->L, sizeof(Lattice)) != 0 || c64->stream != c32->stream)
+        return fail(c64, QCD_EINVAL, "qcd_cg_solve_mixed: need a precision-64 and a precision-32 context on the same lattice and stream");
+    qcd_status s = check_gauge(c64, U64, "qcd_cg_solve_mixed");
+    if (s) return s;
+    if (check_gauge(c32, U32, "qcd_cg_solve_mixed")) return fail(c64, QCD_EINVAL, "qcd_cg_solve_mixed: U32 must be a gauge field of ctx32");
+    if (!b || !x || b->ctx != c64 || x->ctx != c64 || b->kind != QCD_SPINOR_EVEN || x->kind != QCD_SPINOR_EVEN || b->ptr == x->ptr)
+        return fail(c64, QCD_EINVAL, "qcd_cg_solve_mixed: b and x must be distinct QCD_SPINOR_EVEN fields of ctx64");
+    if (!rhs32 || !e32 || rhs32->ctx != c32 || e32->ctx != c32 || rhs32->kind != QCD_SPINOR_EVEN || e32->kind != QCD_SPINOR_EVEN || rhs32->ptr == e32->ptr)
+        return fail(c64, QCD_EINVAL, "qcd_cg_solve_mixed: rhs32 and e32 must be distinct QCD_SPINOR_EVEN fields of ctx32");
+    if (!(m >= 0.0) || !(tol > 0.0) || !(inner_tol > 0.0) || maxiter < 0 || max_outer < 0)
+        return fail(c64, QCD_EINVAL, "qcd_cg_solve_mixed: need m >= 0, tol > 0, inner_tol > 0, maxiter >= 0, max_outer >= 0");
+    if (!c64->ws || !c32->ws) return fail(c64, QCD_EINVAL, "qcd_cg_solve_mixed: both contexts need a workspace (qcd_set_workspace)");
+    if (c64->cg.active || c32->cg.active) return fail(c64, QCD_EINVAL, "qcd_cg_solve_mixed: a CG solve is in progress");
+
+    cudaEvent_t e0, e1;
+    CU(c64, cudaEventCreate(&e0));
+    CU(c64, cudaEventCreate(&e1));
+    cudaEventRecord(e0, c64->stream);
+
+    qcd_mixed_info mi;
+    memset(&mi, 0, sizeof mi);
+    mi.true_resid = 1.0;
+    qcd_status result = QCD_ENOTCONVERGED;
+    const int ncplx = c64->L.Vh * 3;
+    void *r = ws_r(c64), *Mx = ws_Ap(c64);
+    double bb = 0.0, rr = 0.0;
+    int budget = maxiter;
+
+    CU(c64, cudaMemsetAsync(x->ptr, 0, half_spinor_bytes(c64), c64->stream));
+    s = mixed_residual(c64, b->ptr, nullptr, r, &bb);                       // r = b, bb = <b,b>
+    rr = bb;
+    if (!s && bb == 0.0) { mi.converged = 1; mi.true_resid = 0.0; result = QCD_OK; }
+    else if (!s && bb != bb) result = QCD_EBREAKDOWN;
+    else while (!s) {
+        const double rel = sqrt(rr / bb);
+        mi.true_resid = rel;
+        if (rel <= tol) { mi.converged = 1; result = QCD_OK; break; }
+        if (rel != rel) { result = QCD_EBREAKDOWN; break; }
+        if (mi.outer >= max_outer || budget <= 0) break;
+        const double tol_in = inner_tol > 0.5 * tol / rel ? inner_tol : 0.5 * tol / rel;
+        {
+            LaunchScope ls(c64, QCD_K_MISC);                                  // rhs32 = fp32(r / |r|); d_aux->dot holds <r,r>
+            mixed_restrict_kernel<<<(ncplx + 255) / 256, 256, 0, c64->stream>>>(ncplx, (const double2 *)r, (float2 *)rhs32->ptr, c64->d_aux);
+        }
+        qcd_cg_info ii;
+        const qcd_status is = qcd_cg_solve(c32, U32, rhs32, e32, m, tol_in, budget, &ii);
+        if (is != QCD_OK && is != QCD_ENOTCONVERGED) { s = is; if (is == QCD_EBREAKDOWN) { result = is; s = QCD_OK; } break; }
+        budget -= ii.iters; mi.inner_iters += ii.iters; mi.outer += 1;
+        {
+            LaunchScope ls(c64, QCD_K_MISC);                                  // x += |r| fp64(e32)
+            mixed_prolong_kernel<<<(ncplx + 255) / 256, 256, 0, c64->stream>>>(ncplx, (double2 *)x->ptr, (const float2 *)e32->ptr, c64->d_aux);
+        }
+        s = apply_M_raw(c64, U64, Mx, x->ptr, m);                           // r = b - M x in fp64
+        if (s) break;
+        mi.m_applications_fp64 += 1;
+        s = mixed_residual(c64, b->ptr, Mx, r, &rr);
+    }
+    cudaEventRecord(e1, c64->stream);
+    cudaEventSynchronize(e1);
+    float ms = 0.f;
+    cudaEventElapsedTime(&ms, e0, e1);
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    mi.seconds = ms * 1e-3;
+    if (info) *info = mi;
+    if (s) { if (s != QCD_ECUDA || c64->err.empty()) fail(c64, s, "qcd_cg_solve_mixed: inner solve failed: %s", qcd_last_error(c32)); return s; }
+    if (result == QCD_ENOTCONVERGED) return fail(c64, result, "qcd_cg_solve_mixed: not converged");
+    if (result == QCD_EBREAKDOWN) return fail(c64, result, "qcd_cg_solve_mixed: breakdown");
+    return QCD_OK;
 }

@@ -13,7 +13,10 @@
 
 namespace qcd {
 
-// CG recurrence state, resident on the device (north_star (d)).
+// Largest number of right-hand sides handled by one launch (NMULTI).
+enum { MAXRHS = 8 };
+
+// CG recurrence state, resident on the device (north_star (d)); one per right-hand side.
 struct CgScalars {
     double rr;        // <r,r> of the current residual
     double bb;        // <b,b>
@@ -59,6 +62,36 @@ __device__ __forceinline__ bool publish_partial(double v, double *partials, unsi
     const double s = block_sum<BLOCK>(v, smem);
     if (threadIdx.x == 0) {
         partials[blockIdx.x] = s;
+        __threadfence();
+        const unsigned t = atomicInc(ticket, gridDim.x - 1);
+        *smem_flag = (t == gridDim.x - 1);
+    }
+    __syncthreads();
+    return *smem_flag != 0;
+}
+
+// Stage 1 + ticket for N sums at once (multiple right-hand sides): sum r of
+// this block goes to partials[r * stride + blockIdx.x]; ONE ticket serves all N.  For N = 1
+// the summation order is that of publish_partial.  smem holds N * BLOCK/32 doubles.
+template <int BLOCK, int N>
+__device__ __forceinline__ bool publish_partials(const double (&v)[N], double *partials, size_t stride,
+                                                 unsigned *ticket, double *smem, int *smem_flag)
+{
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+#pragma unroll
+    for (int r = 0; r < N; ++r) {
+        const double s = warp_sum(v[r]);
+        if (lane == 0) smem[r * (BLOCK / 32) + w] = s;
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+#pragma unroll
+        for (int r = 0; r < N; ++r) {
+            double s = 0.0;
+#pragma unroll
+            for (int i = 0; i < BLOCK / 32; ++i) s += smem[r * (BLOCK / 32) + i];
+            partials[(size_t)r * stride + blockIdx.x] = s;
+        }
         __threadfence();
         const unsigned t = atomicInc(ticket, gridDim.x - 1);
         *smem_flag = (t == gridDim.x - 1);

@@ -22,6 +22,21 @@ def test_byte_and_flop_model():
     assert abs(570 / (126 * 8) - 0.57) < 0.01 and abs(570 / (126 * 4) - 1.13) < 0.01
 
 
+def test_variant_byte_model_matches_the_papers_formula():
+    """two rows + temporal gauge, n vectors: AI(n) = n 570 / (8 (6 12 + n 9 6)) in fp64."""
+    import bench
+    for n in (1, 2, 3, 4, 6, 8, 16):
+        comp, nom = bench.variant_reals(2, 1, n, 10 ** 9)           # N3 -> infinity: exactly 6 links per site
+        assert abs(nom - (6 * 12 + n * 9 * 6)) < 1e-6
+        assert abs(570 * n / (nom * 8) - n * 570 / (8 * (6 * 12 + n * 9 * 6))) < 1e-8
+        assert abs(comp - (72 + 12 * n)) < 1e-6
+    assert bench.variant_reals(2, 1, 1, 10 ** 9)[1] == pytest.approx(126)            # "a total float count of 126 per site"
+    assert bench.variant_reals(3, 0, 1, 64) == (bench.REALS_DSLASH_COMPULSORY, bench.REALS_DSLASH_NOMINAL)
+    assert bench.variant_reals(2, 0, 1, 64) == (108, 150)                              # SURVEY.md Sec. 8(d)
+    # the slices x3 = 0 / 1 still read their time links: 2 / N3 links per site on average
+    assert bench.variant_reals(2, 1, 1, 64)[0] == pytest.approx((6 + 2 / 64) * 12 + 12)
+
+
 _WORKER = r"""
 import os, sys
 sys.path.insert(0, {root!r})

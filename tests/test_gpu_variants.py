@@ -1,0 +1,379 @@
+"""GPU parity of the paper's Dslash variants and of
+the mixed-precision solver against oracle/variants.py, through the C-ABI, on the same seeded inputs.
+
+  two-row links    the kernel rebuilds row 2 = conj(row 0 x row 1) from the STORED rows, so the
+                   reference is the oracle applied to reconstruct12(compress12(U as stored))
+  temporal gauge   device transform vs oracle transform (U', g); the TG kernel (time links with
+                   x3 != 0 never read) vs the oracle on the fixed links; covariance back to D[U]
+  several vectors  every vector of a multi call vs the oracle applied to it alone; n lock-step CG
+                   solves vs n oracle solves
+  mixed precision  defect-correction CG vs oracle.variants.mixed_cg: fp64 true residual <= tol
+
+Tolerances as in test_gpu_parity.py (north_star): 1e-13 (fp64), 2e-6 (fp32), per-site measure R10."""
+import numpy as np
+import pytest
+
+import oracle
+import oracle.variants as ov
+import qcd_inputs
+from util import DSLASH_TOL, dslash_rel_err, iters_close
+
+pytestmark = pytest.mark.gpu
+
+LATTICES = [
+    ((4, 4, 4, 4), "haar", None),
+    ((4, 6, 2, 8), "haar", None),            # N2 = 2
+    ((8, 4, 6, 10), "near_identity", 0.5),   # several blocks and a ragged tail
+    ((12, 2, 2, 4), "haar", None),           # time slices shorter than a warp: x3 varies inside a warp
+    ((16, 16, 16, 16), "near_identity", 0.3),
+]
+
+
+@pytest.fixture(scope="module")
+def q():
+    import paper_2502_03249_b200 as pkg
+    return pkg
+
+
+def _rounded(a, prec):
+    return a if prec == 64 else a.astype(np.complex64).astype(np.complex128)
+
+
+def _full_dslash(ctx, q, fU, phi):
+    """D phi on the full lattice through qcd_dslash_eo + qcd_dslash_oe."""
+    fphi = ctx.field(q.QCD_SPINOR_FULL).upload(phi)
+    fout = ctx.field(q.QCD_SPINOR_FULL)
+    fout.buf.zero_()
+    ctx.qcd_dslash_eo(fU, fout, fphi)
+    ctx.qcd_dslash_oe(fU, fout, fphi)
+    return fout.download()
+
+
+def _check_full(dims, got, ref, tol, what=""):
+    par = qcd_inputs.site_parity(dims)
+    for p in (0, 1):
+        err = dslash_rel_err(got[par == p], ref[par == p])
+        assert err <= tol, (what, p, err)
+
+
+# ------------------------------------------------------------------------------------------
+# two-row links
+# ------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("prec", [64, 32])
+@pytest.mark.parametrize("dims,links,eps", LATTICES)
+def test_two_row_links(q, dims, links, eps, prec):
+    ctx = q.Context(dims, prec)
+    U = qcd_inputs.gauge_field(dims, links, seed=0, eps=eps)
+    phi = qcd_inputs.gaussian_spinor(dims, seed=1)
+    Ur, phir = _rounded(U, prec), _rounded(phi, prec)
+    Urec = ov.reconstruct12(ov.compress12(Ur))               # what a two-row field represents
+
+    f12 = ctx.field(q.QCD_GAUGE_2ROW).upload(U)
+    back = f12.download().astype(np.complex128)
+    assert np.array_equal(back[:, :, :2, :], Ur[:, :, :2, :])            # stored rows: exact
+    eps_m = 1e-15 if prec == 64 else 5e-7
+    assert np.max(np.abs(back - Urec)) <= 8 * eps_m                       # rebuilt row
+    assert np.max(np.abs(Urec - Ur)) <= (1e-14 if prec == 64 else 1e-6)   # the inputs are SU(3)
+
+    # device-side compression gives the same planes as the direct upload
+    fU = ctx.field(q.QCD_GAUGE).upload(U)
+    g12 = ctx.field(q.QCD_GAUGE_2ROW)
+    ctx.qcd_gauge_compress(fU, g12)
+    import torch
+    torch.cuda.synchronize()
+    assert torch.equal(g12.buf, f12.buf)
+
+    got = _full_dslash(ctx, q, f12, phi)
+    _check_full(dims, got, oracle.dslash(dims, Urec, phir, -1), DSLASH_TOL[prec], "two-row vs oracle on rebuilt links")
+    if prec == 64:      # and the rebuilt links are the links: same answer as Eq. (1) on U itself
+        _check_full(dims, got, oracle.dslash(dims, U, phi, -1), DSLASH_TOL[64], "two-row vs oracle on full links")
+    ctx.close()
+
+
+@pytest.mark.parametrize("prec", [64, 32])
+def test_two_row_apply_M_and_cg(q, prec):
+    dims, m = (8, 4, 6, 10), 0.1
+    tol = 1e-10 if prec == 64 else 1e-5
+    ctx = q.Context(dims, prec)
+    U = qcd_inputs.gauge_field(dims, "near_identity", seed=0, eps=0.5)
+    b = qcd_inputs.gaussian_source(dims, seed=1)
+    Ur, br = _rounded(U, prec), _rounded(b, prec)
+    Urec = ov.reconstruct12(ov.compress12(Ur))
+    par = qcd_inputs.site_parity(dims)
+    f12 = ctx.field(q.QCD_GAUGE_2ROW).upload(U)
+    fb = ctx.field(q.QCD_SPINOR_EVEN).upload(b)
+    fx = ctx.field(q.QCD_SPINOR_EVEN)
+    ctx.qcd_apply_M(f12, fx, fb, m)
+    got = fx.download()
+    assert dslash_rel_err(got[par == 0], oracle.apply_M(dims, Urec, br, m)[par == 0]) <= DSLASH_TOL[prec]
+    info = ctx.qcd_cg_solve(f12, fb, fx, m, tol, 5000)
+    x = fx.download().astype(np.complex128)
+    _, oinfo = oracle.cg(dims, Urec.astype(ctx.cdtype), br.astype(ctx.cdtype), m, tol, 5000)
+    assert info["converged"] and iters_close(info["iters"], oinfo["iters"]), (info, oinfo)
+    assert oracle.true_residual(dims, Urec, br, x, m) <= tol * (1.0 if prec == 64 else 1.5)
+    ctx.close()
+
+
+# ------------------------------------------------------------------------------------------
+# temporal gauge (reading R20)
+# ------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("dims,links,eps", LATTICES)
+def test_temporal_gauge_transform_fp64(q, dims, links, eps):
+    ctx = q.Context(dims, 64)
+    U = qcd_inputs.gauge_field(dims, links, seed=0, eps=eps)
+    phi = qcd_inputs.gaussian_spinor(dims, seed=1)
+    Ufix_ref, g_ref = ov.temporal_gauge(dims, U)
+    fU = ctx.field(q.QCD_GAUGE).upload(U)
+    fUf = ctx.field(q.QCD_GAUGE)
+    fg = ctx.field(q.QCD_COLOUR_MATRIX)
+    ctx.qcd_gauge_fix_temporal(fU, fUf, fg)
+    g = fg.download()
+    Ufix = fUf.download()
+    assert np.max(np.abs(g - g_ref)) <= 1e-13
+    assert np.max(np.abs(Ufix - Ufix_ref)) <= 1e-13
+    x3 = qcd_inputs.site_coords(dims)[:, 3]
+    assert np.array_equal(Ufix[x3 != 0, 3], np.broadcast_to(np.eye(3), Ufix[x3 != 0, 3].shape))   # exactly 1
+    assert np.max(np.abs(Ufix[x3 == 0, 3] - np.eye(3))) > 1e-3                                      # the Polyakov loop is not
+
+    # rotation g phi, and back
+    fphi = ctx.field(q.QCD_SPINOR_FULL).upload(phi)
+    frot = ctx.field(q.QCD_SPINOR_FULL)
+    ctx.qcd_spinor_rotate(fg, frot, fphi, dagger=False)
+    rot = frot.download()
+    assert np.max(np.abs(rot - ov.rotate_spinor(g_ref, phi))) <= 1e-13
+    ctx.qcd_spinor_rotate(fg, frot, frot, dagger=True)              # in place
+    assert np.max(np.abs(frot.download() - phi)) <= 1e-13
+
+    # the TG kernel on the fixed links (it never reads the unit time links) ...
+    got = _full_dslash(ctx, q, fUf, rot)
+    _check_full(dims, got, oracle.dslash(dims, Ufix_ref, ov.rotate_spinor(g_ref, phi), -1), DSLASH_TOL[64], "TG kernel")
+    # ... is gauge covariant: g^dagger D[U'] g phi = D[U] phi
+    fgot = ctx.field(q.QCD_SPINOR_FULL).upload(got)
+    ctx.qcd_spinor_rotate(fg, fgot, fgot, dagger=True)
+    _check_full(dims, fgot.download(), oracle.dslash(dims, U, phi, -1), DSLASH_TOL[64], "covariance")
+
+    # two rows + temporal gauge: the paper's 126-real kernel
+    f12 = ctx.field(q.QCD_GAUGE_2ROW)
+    ctx.qcd_gauge_compress(fUf, f12)
+    got12 = _full_dslash(ctx, q, f12, rot)
+    _check_full(dims, got12, oracle.dslash(dims, Ufix_ref, ov.rotate_spinor(g_ref, phi), -1), DSLASH_TOL[64], "two-row + TG")
+    ctx.close()
+
+
+def test_temporal_gauge_kernel_does_not_read_unit_links(q):
+    """Poison the time links with x3 != 0 after marking the field: the result must not change."""
+    dims = (8, 4, 6, 10)
+    ctx = q.Context(dims, 64)
+    U = qcd_inputs.gauge_field(dims, "haar", seed=0)
+    phi = qcd_inputs.gaussian_spinor(dims, seed=1)
+    Ufix, _ = ov.temporal_gauge(dims, U)
+    x3 = qcd_inputs.site_coords(dims)[:, 3]
+    poisoned = Ufix.copy()
+    poisoned[x3 != 0, 3] = np.nan
+    for kind in (q.QCD_GAUGE, q.QCD_GAUGE_2ROW):
+        f = ctx.field(kind).upload(poisoned)
+        ctx.qcd_gauge_set_temporal_unit(f, True)
+        got = _full_dslash(ctx, q, f, phi)
+        assert np.isfinite(got).all()
+        _check_full(dims, got, oracle.dslash(dims, Ufix, phi, -1), DSLASH_TOL[64], kind)
+        ctx.qcd_gauge_set_temporal_unit(f, False)
+        assert not np.isfinite(_full_dslash(ctx, q, f, phi)).all()
+    ctx.close()
+
+
+@pytest.mark.parametrize("dims,links,eps", LATTICES[1:4])
+def test_temporal_gauge_fp32(q, dims, links, eps):
+    """fp32: the links fixed by the oracle in fp64, rounded, uploaded and marked; reference = oracle on
+    the rounded links with the unit time links exactly 1."""
+    ctx = q.Context(dims, 32)
+    U = qcd_inputs.gauge_field(dims, links, seed=0, eps=eps)
+    phi = qcd_inputs.gaussian_spinor(dims, seed=1)
+    Ufix, _ = ov.temporal_gauge(dims, U)
+    x3 = qcd_inputs.site_coords(dims)[:, 3]
+    Ufix[x3 != 0, 3] = np.eye(3)
+    Ur, phir = _rounded(Ufix, 32), _rounded(phi, 32)
+    for kind in (q.QCD_GAUGE, q.QCD_GAUGE_2ROW):
+        f = ctx.field(kind).upload(Ufix)
+        ctx.qcd_gauge_set_temporal_unit(f, True)
+        ref_links = Ur if kind == q.QCD_GAUGE else ov.reconstruct12(ov.compress12(Ur))
+        _check_full(dims, _full_dslash(ctx, q, f, phi), oracle.dslash(dims, ref_links, phir, -1), DSLASH_TOL[32], kind)
+    ctx.close()
+
+
+def test_temporal_gauge_cg_returns_rotated_solution(q):
+    """M[U'] x' = g b  is solved by  x' = g x  (SURVEY.md pin P4)."""
+    dims, m, tol = (8, 4, 6, 10), 0.1, 1e-10
+    ctx = q.Context(dims, 64)
+    U = qcd_inputs.gauge_field(dims, "near_identity", seed=0, eps=0.5)
+    b = qcd_inputs.gaussian_source(dims, seed=1)
+    fU = ctx.field(q.QCD_GAUGE).upload(U)
+    fUf, fg = ctx.field(q.QCD_GAUGE), ctx.field(q.QCD_COLOUR_MATRIX)
+    ctx.qcd_gauge_fix_temporal(fU, fUf, fg)
+    f12 = ctx.field(q.QCD_GAUGE_2ROW)
+    ctx.qcd_gauge_compress(fUf, f12)
+    fb = ctx.field(q.QCD_SPINOR_EVEN).upload(b)
+    fbr, fx = ctx.field(q.QCD_SPINOR_EVEN), ctx.field(q.QCD_SPINOR_EVEN)
+    ctx.qcd_spinor_rotate(fg, fbr, fb)
+    info = ctx.qcd_cg_solve(f12, fbr, fx, m, tol, 5000)
+    ctx.qcd_spinor_rotate(fg, fx, fx, dagger=True)
+    x = fx.download()
+    _, oinfo = oracle.cg(dims, U, b, m, tol, 5000)
+    assert info["converged"] and iters_close(info["iters"], oinfo["iters"])
+    assert oracle.true_residual(dims, U, b, x, m) <= tol
+    ctx.close()
+
+
+# ------------------------------------------------------------------------------------------
+# several vectors per link load (NMULTI)
+# ------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("prec", [64, 32])
+@pytest.mark.parametrize("n", [1, 2, 3, 4, 5, 6, 7, 8])
+@pytest.mark.parametrize("kind_name,tg", [("QCD_GAUGE", False), ("QCD_GAUGE_2ROW", True)])
+def test_dslash_multi(q, n, prec, kind_name, tg):
+    dims = (8, 4, 6, 10)
+    kind = getattr(q, kind_name)
+    ctx = q.Context(dims, prec)
+    U = qcd_inputs.gauge_field(dims, "haar", seed=0)
+    if tg:
+        U, _ = ov.temporal_gauge(dims, U)
+        U[qcd_inputs.site_coords(dims)[:, 3] != 0, 3] = np.eye(3)
+    Ur = _rounded(U, prec)
+    if kind == q.QCD_GAUGE_2ROW:
+        Ur = ov.reconstruct12(ov.compress12(Ur))
+    fU = ctx.field(kind).upload(U)
+    ctx.qcd_gauge_set_temporal_unit(fU, tg)
+    phis = [qcd_inputs.gaussian_spinor(dims, seed=10 + i) for i in range(n)]
+    par = qcd_inputs.site_parity(dims)
+    fin = [ctx.field(q.QCD_SPINOR_FULL).upload(p) for p in phis]
+    fout = [ctx.field(q.QCD_SPINOR_FULL) for _ in range(n)]
+    for f in fout:
+        f.buf.zero_()
+    ctx.qcd_dslash_eo_multi(fU, fout, fin)
+    ctx.qcd_dslash_oe_multi(fU, fout, fin)
+    refs = ov.dslash_multi(dims, Ur, [_rounded(p, prec) for p in phis], -1)
+    for i in range(n):
+        got = fout[i].download()
+        for p in (0, 1):
+            assert dslash_rel_err(got[par == p], refs[i][par == p]) <= DSLASH_TOL[prec], (i, p)
+    ctx.close()
+
+
+@pytest.mark.parametrize("prec,n", [(64, 2), (64, 3), (64, 8), (32, 4)])
+def test_cg_multi_is_n_independent_solves(q, prec, n):
+    dims, m = (8, 4, 6, 10), 0.1
+    tol = 1e-10 if prec == 64 else 1e-5
+    ctx = q.Context(dims, prec, nrhs=n)
+    U = qcd_inputs.gauge_field(dims, "near_identity", seed=0, eps=0.5)
+    Ur = _rounded(U, prec)
+    bs = [qcd_inputs.gaussian_source(dims, seed=20 + i) * (10.0 ** (i - 1)) for i in range(n)]
+    bs[1] = np.zeros_like(bs[1])                                  # a zero source: converged at once, x = 0
+    fU = ctx.field(q.QCD_GAUGE).upload(U)
+    fb = [ctx.field(q.QCD_SPINOR_EVEN).upload(b) for b in bs]
+    fx = [ctx.field(q.QCD_SPINOR_EVEN) for _ in range(n)]
+    infos = ctx.qcd_cg_solve_multi(fU, fb, fx, m, tol, 5000)
+    _, oinfos = ov.cg_multi(dims, Ur.astype(ctx.cdtype), [_rounded(b, prec).astype(ctx.cdtype) for b in bs], m, tol, 5000)
+    single = q.Context(dims, prec)
+    sU = single.field(q.QCD_GAUGE).upload(U)
+    for i in range(n):
+        x = fx[i].download().astype(np.complex128)
+        assert infos[i]["converged"], (i, infos[i])
+        assert iters_close(infos[i]["iters"], oinfos[i]["iters"]), (i, infos[i], oinfos[i])
+        if not bs[i].any():
+            assert infos[i]["iters"] == 0 and not x.any()
+            continue
+        assert oracle.true_residual(dims, Ur, _rounded(bs[i], prec), x, m) <= tol * (1.0 if prec == 64 else 1.5), i
+        # identical to the single-vector solve: same arithmetic, same reduction order
+        sb, sx = single.field(q.QCD_SPINOR_EVEN).upload(bs[i]), single.field(q.QCD_SPINOR_EVEN)
+        sinfo = single.qcd_cg_solve(sU, sb, sx, m, tol, 5000)
+        assert sinfo["iters"] == infos[i]["iters"], (i, sinfo, infos[i])
+        assert np.allclose(sx.download(), fx[i].download(), rtol=0, atol=1e-12 * np.max(np.abs(x)) if prec == 64 else 1e-5 * np.max(np.abs(x)))
+    single.close()
+    ctx.close()
+
+
+def test_multi_argument_errors(q):
+    dims = (4, 4, 4, 4)
+    ctx = q.Context(dims, 64)            # workspace for ONE right-hand side only
+    fU = ctx.field(q.QCD_GAUGE).upload(qcd_inputs.gauge_field(dims, "haar", seed=0))
+    fb = [ctx.field(q.QCD_SPINOR_EVEN).upload(qcd_inputs.gaussian_source(dims, seed=i)) for i in range(2)]
+    fx = [ctx.field(q.QCD_SPINOR_EVEN) for _ in range(2)]
+    with pytest.raises(q.QcdError) as e:
+        ctx.qcd_cg_solve_multi(fU, fb, fx, 0.1, 1e-8, 100)
+    assert e.value.status == q.QCD_EINVAL and "workspace" in str(e.value)
+    with pytest.raises(q.QcdError):
+        ctx.qcd_cg_solve_multi(fU, fb, [fx[0], fx[0]], 0.1, 1e-8, 100)       # aliased solutions
+    fo = [ctx.field(q.QCD_SPINOR_ODD) for _ in range(9)]
+    with pytest.raises(q.QcdError):
+        ctx.qcd_dslash_oe_multi(fU, fo, [fb[0]] * 9)                          # n > QCD_MAX_RHS
+    with pytest.raises(q.QcdError):
+        ctx.qcd_dslash_eo_multi(fU, fx, fb)                                   # parity mismatch
+    ctx.close()
+
+
+# ------------------------------------------------------------------------------------------
+# precision conversion and mixed-precision defect-correction CG (reading R21)
+# ------------------------------------------------------------------------------------------
+def test_field_convert_rounds_to_nearest(q):
+    dims = (8, 4, 6, 10)
+    c64, c32 = q.Context(dims, 64), q.Context(dims, 32)
+    U = qcd_inputs.gauge_field(dims, "haar", seed=0)
+    for kind in (q.QCD_GAUGE, q.QCD_GAUGE_2ROW):
+        f64 = c64.field(kind).upload(U)
+        f32 = c32.field(kind)
+        c64.qcd_field_convert(f32, f64)
+        direct = c32.field(kind).upload(U)          # host-side rounding by numpy astype
+        import torch
+        torch.cuda.synchronize()
+        assert torch.equal(f32.buf, direct.buf)
+    c64.close(); c32.close()
+
+
+@pytest.mark.parametrize("dims,links,eps,m,tol", [
+    ((8, 4, 6, 10), "haar", None, 0.1, 1e-10),
+    ((8, 8, 8, 8), "haar", None, 0.05, 1e-9),
+    ((16, 16, 16, 16), "near_identity", 0.3, 0.05, 1e-10),
+])
+def test_mixed_precision_cg(q, dims, links, eps, m, tol):
+    inner_tol, maxiter = 1e-3, 20000
+    c64, c32 = q.Context(dims, 64), q.Context(dims, 32)
+    U = qcd_inputs.gauge_field(dims, links, seed=0, eps=eps)
+    b = qcd_inputs.gaussian_source(dims, seed=1)
+    U64 = c64.field(q.QCD_GAUGE).upload(U)
+    U32 = c32.field(q.QCD_GAUGE)
+    c64.qcd_field_convert(U32, U64)
+    fb, fx = c64.field(q.QCD_SPINOR_EVEN).upload(b), c64.field(q.QCD_SPINOR_EVEN)
+    rhs32, e32 = c32.field(q.QCD_SPINOR_EVEN), c32.field(q.QCD_SPINOR_EVEN)
+    info = c64.qcd_cg_solve_mixed(c32, U64, U32, fb, fx, rhs32, e32, m, tol, inner_tol, maxiter)
+    x = fx.download()
+    xo, oinfo = ov.mixed_cg(dims, U, b, m, tol, inner_tol, maxiter)
+    assert info["converged"] and oinfo["converged"], (info, oinfo)
+    true = oracle.true_residual(dims, U, b, x, m)
+    assert true <= tol, true                                             # north_star: fp64 true residual <= tol
+    assert abs(true - info["true_resid"]) <= 1e-3 * tol + 1e-14          # the device-side residual is the true one
+    assert abs(info["outer"] - oinfo["outer"]) <= 1, (info, oinfo)
+    assert iters_close(info["inner_iters"], oinfo["inner_iters"]) or abs(info["outer"] - oinfo["outer"]) == 1, (info, oinfo)
+    assert info["m_applications_fp64"] == info["outer"]
+    # the same x as the oracle's up to the conditioning of M:  |dx| / |x| <= kappa * tol, kappa <= (m^2 + 64) / m^2
+    kappa = (m * m + 64.0) / (m * m)
+    assert np.linalg.norm(x - xo) / np.linalg.norm(xo) <= kappa * tol
+    # and cheaper than it looks: the fp64 work is `outer` operator applications
+    assert info["outer"] <= 12
+    c64.close(); c32.close()
+
+
+def test_mixed_zero_source_and_budget(q):
+    dims = (4, 4, 4, 4)
+    c64, c32 = q.Context(dims, 64), q.Context(dims, 32)
+    U = qcd_inputs.gauge_field(dims, "haar", seed=0)
+    U64 = c64.field(q.QCD_GAUGE).upload(U)
+    U32 = c32.field(q.QCD_GAUGE).upload(U)
+    fb, fx = c64.field(q.QCD_SPINOR_EVEN), c64.field(q.QCD_SPINOR_EVEN)
+    fb.buf.zero_()
+    fx.buf.fill_(7)
+    rhs32, e32 = c32.field(q.QCD_SPINOR_EVEN), c32.field(q.QCD_SPINOR_EVEN)
+    info = c64.qcd_cg_solve_mixed(c32, U64, U32, fb, fx, rhs32, e32, 0.1, 1e-10, 1e-3, 100)
+    assert info["converged"] and info["outer"] == 0 and not fx.download().any()
+    fb.upload(qcd_inputs.gaussian_source(dims, seed=1))
+    info = c64.qcd_cg_solve_mixed(c32, U64, U32, fb, fx, rhs32, e32, 0.1, 1e-10, 1e-3, 10)     # budget of 10 inner iterations
+    assert info["status"] == q.QCD_ENOTCONVERGED and not info["converged"] and info["inner_iters"] == 10
+    c64.close(); c32.close()
