@@ -61,6 +61,11 @@ def parse_args():
     ap.add_argument("--impl", default="ours", choices=("ours", "reference"))
     ap.add_argument("--lattice", default=None, help="override dims, e.g. 16,16,16,16 (testing only)")
     ap.add_argument("--quick", action="store_true", help="skip the extra reports (full solves, fp32, cpu_baseline)")
+    ap.add_argument("--variants-only", action="store_true",
+                    help="run only the Dslash variant sweep (two-row / temporal gauge / NMULTI) and print it; used for ncu captures")
+    ap.add_argument("--prec", type=int, default=64, choices=(64, 32), help="precision of --variants-only")
+    ap.add_argument("--nmulti", default="1,2,3,4,6,8", help="NMULTI values of --variants-only")
+    ap.add_argument("--reps", type=int, default=10, help="timed launches per variant of --variants-only")
     return ap.parse_args()
 
 
@@ -195,7 +200,7 @@ def variant_reals(nrow, tg, n, N3):
 
 
 def time_dslash_multi(torch, ctx, fU, fins, fouts, reps=10):
-    for _ in range(2):
+    for _ in range(2 if reps > 1 else 0):
         ctx.qcd_dslash_oe_multi(fU, fouts, fins)
     torch.cuda.synchronize()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -207,7 +212,7 @@ def time_dslash_multi(torch, ctx, fU, fins, fouts, reps=10):
     return e0.elapsed_time(e1) / reps
 
 
-def variants_sweep(q, torch, ctx, fU_full, dims, peak, nmulti=(1, 2, 3, 4, 6, 8)):
+def variants_sweep(q, torch, ctx, fU_full, dims, peak, nmulti=(1, 2, 3, 4, 6, 8), reps=10):
     """Dslash with the paper's traffic reductions, reported separately from the headline:
     link storage x temporal gauge x NMULTI.  Throughput does not depend on the link values, so the
     temporal-gauge rows run on the same links with the field marked (the kernel then skips the time links
@@ -227,7 +232,7 @@ def variants_sweep(q, torch, ctx, fU_full, dims, peak, nmulti=(1, 2, 3, 4, 6, 8)
     for name, fU, nrow, tg in (("full18", fU_full, 3, 0), ("tworow12", f12, 2, 0), ("tworow12+temporal_gauge", f12, 2, 1)):
         ctx.qcd_gauge_set_temporal_unit(fU, bool(tg))
         for n in nmulti:
-            ms = time_dslash_multi(torch, ctx, fU, fins[:n], fouts[:n])
+            ms = time_dslash_multi(torch, ctx, fU, fins[:n], fouts[:n], reps)
             comp, nom = variant_reals(nrow, tg, n, dims[3])
             gbs = comp * rsize * Vh / ms / 1e6
             rows.append({"links": name, "nmulti": n, "ms": round(ms, 5),
@@ -278,6 +283,32 @@ def cg_multi_report(q, torch, device, dims, prec, fU_full, m, ns=(1, 2, 4), iter
         ctx.close()
         torch.cuda.empty_cache()
     return rows
+
+
+def small_lattice_report(q, torch, device):
+    """configs[1] (16^4, links fit the L2): the solve is launch- and reduction-latency bound (PAPER.md:54);
+    kernel-by-kernel enqueue on the default stream vs CUDA-graph replay of 16 iterations on a side stream."""
+    import contextlib
+    dims = (16, 16, 16, 16)
+    cfg, U, b = make_inputs(dims, 1)
+    rows = []
+    for name, side in (("kernel-by-kernel enqueue (default stream)", False), ("CUDA-graph replay, 16 iterations per launch (side stream)", True)):
+        stream = torch.cuda.Stream(device=device) if side else None
+        with (torch.cuda.stream(stream) if side else contextlib.nullcontext()):
+            for prec, tol in ((64, cfg["tol64"]), (32, cfg["tol32"])):
+                ctx = q.Context(dims, prec, stream=stream, device=device)
+                fU = ctx.field(q.QCD_GAUGE).upload(U)
+                fb = ctx.field(q.QCD_SPINOR_EVEN).upload(b)
+                fx = ctx.field(q.QCD_SPINOR_EVEN)
+                ctx.qcd_cg_solve(fU, fb, fx, cfg["m"], tol, cfg["maxiter"])
+                t0 = time.perf_counter()
+                info = ctx.qcd_cg_solve(fU, fb, fx, cfg["m"], tol, cfg["maxiter"])
+                wall = time.perf_counter() - t0
+                rows.append({"loop": name, "prec": prec, "tol": tol, "iters": info["iters"], "converged": info["converged"],
+                             "ms_per_solve_device": round(1e3 * info["seconds"], 4), "ms_per_solve_wall": round(1e3 * wall, 4),
+                             "us_per_iter": round(1e6 * info["seconds"] / max(info["iters"], 1), 3)})
+                ctx.close()
+    return {"lattice": list(dims), "rows": rows}
 
 
 def dslash_report(ms, Vh, rsize, peak):
@@ -493,6 +524,7 @@ def extras(args, q, torch, ctx, out, cfg, dims, U, b, fU, fb, fx, fo, peak):
             t2[f"fp{prec}"] = variants_sweep(q, torch, c, f, d32, peak)
             f.free(); c.close()
         out["variants_table2_32x32x32x32"] = t2
+        out["cg_small_lattice"] = small_lattice_report(q, torch, ctx.device)
     out["paper_context"] = {"A100_OpenCL_dslash_fp64_TFLOPs_32^4_12real_links_gaugefixed": 1.245,
                             "A100_OpenCL_cg_update_GBs_48^4_fp64": 1351, "source": "PAPER.md:59,87 (other hardware; context only)"}
 
@@ -526,9 +558,25 @@ def run_reference(args):
     print(json.dumps(out), flush=True)
 
 
+def run_variants_only(args):
+    """Dslash variant sweep alone (rank 0, one GPU): `--lattice`, `--prec`, `--nmulti`, `--reps`."""
+    import torch
+    import paper_2502_03249_b200 as q
+    dims = tuple(int(v) for v in args.lattice.split(",")) if args.lattice else (64, 64, 64, 64)
+    peak, _ = load_peaks()
+    _, U, _ = make_inputs(dims)
+    ctx = q.Context(dims, args.prec)
+    fU = ctx.field(q.QCD_GAUGE).upload(U)
+    rows = variants_sweep(q, torch, ctx, fU, dims, peak, tuple(int(v) for v in args.nmulti.split(",")), args.reps)
+    print(json.dumps({"variants": rows, "lattice": list(dims), "prec": args.prec, "gpu_launches": ctx.qcd_launch_count()}), flush=True)
+    ctx.close()
+
+
 def main():
     args = parse_args()
-    if args.impl == "reference":
+    if args.variants_only:
+        run_variants_only(args)
+    elif args.impl == "reference":
         run_reference(args)
     else:
         run_ours(args)

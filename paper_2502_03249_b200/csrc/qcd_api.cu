@@ -46,6 +46,7 @@ struct CgState {
     double m, tol;
     int maxiter;
     cudaEvent_t ev_begin, ev_end;
+    cudaGraphExec_t graph;    // replayed by cg_run on small lattices; destroyed by qcd_cg_finish after its sync
 };
 
 struct qcd_ctx {
@@ -648,6 +649,7 @@ extern "C" qcd_status qcd_cg_finish_multi(qcd_ctx *ctx, qcd_cg_info *info)
     CU(ctx, cudaEventRecord(ctx->cg.ev_end, ctx->stream));
     const CgScalars *s;
     qcd_status st = read_scalars(ctx, &s);
+    if (ctx->cg.graph) { cudaGraphExecDestroy(ctx->cg.graph); ctx->cg.graph = nullptr; }
     if (st) return st;
     float ms = 0.f;
     CU(ctx, cudaEventElapsedTime(&ms, ctx->cg.ev_begin, ctx->cg.ev_end));
@@ -670,6 +672,33 @@ extern "C" qcd_status qcd_cg_finish(qcd_ctx *ctx, qcd_cg_info *info)
     return qcd_cg_finish_multi(ctx, info);
 }
 
+// Small lattices: an iteration is 4 kernels of a few microseconds each, so the host's launch rate,
+// not the device, bounds the solve ("global reductions which have higher latencies ... more
+// pronounced for smaller lattice sizes").  There the loop replays a CUDA graph of
+// GRAPH_ITERS iterations (one launch per 4 * GRAPH_ITERS kernels).  The pointers of a solve are
+// fixed and alpha, beta, the flags live on the device, so one capture serves the whole solve.
+// Capture needs a non-default stream; on the legacy default stream, or while per-launch
+// profiling is on, the plain loop below is used.
+enum { GRAPH_ITERS = 16, GRAPH_MAX_VH = 1 << 21 };
+
+static cudaGraphExec_t cg_capture_graph(qcd_ctx *ctx)
+{
+    if (ctx->L.Vh > GRAPH_MAX_VH || ctx->prof_on || ctx->stream == nullptr || ctx->cg.maxiter < GRAPH_ITERS) return nullptr;
+    if (cudaStreamBeginCapture(ctx->stream, cudaStreamCaptureModeThreadLocal) != cudaSuccess) { cudaGetLastError(); return nullptr; }
+    const long long l0 = ctx->launches;
+    const qcd_status s = qcd_cg_iterate(ctx, GRAPH_ITERS);
+    ctx->launches = l0;
+    cudaGraph_t graph = nullptr;
+    cudaGraphExec_t exec = nullptr;
+    const cudaError_t e = cudaStreamEndCapture(ctx->stream, &graph);
+    if (s == QCD_OK && e == cudaSuccess && graph) {
+        if (cudaGraphInstantiate(&exec, graph, 0) != cudaSuccess) exec = nullptr;
+    }
+    if (graph) cudaGraphDestroy(graph);
+    cudaGetLastError();
+    return exec;
+}
+
 // Host loop: keep two chunks of iterations in flight; after each chunk the scalars are copied
 // to pinned memory and an event is recorded, and the host waits on the OLDER chunk's event
 // only, so the device never idles while the host decides.  Iterations enqueued after the
@@ -679,24 +708,42 @@ static qcd_status cg_run(qcd_ctx *ctx)
     const int maxiter = ctx->cg.maxiter, n = ctx->cg.n;
     int enq = 0, head = 0, tail = 0, pending = 0, chunk = 8;
     bool first = true;
+    cudaGraphExec_t graph = cg_capture_graph(ctx);
+    ctx->cg.graph = graph;
+    if (graph) chunk = GRAPH_ITERS;
+    qcd_status result = QCD_OK;
     for (;;) {
         while (pending < POLL_SLOTS && (enq < maxiter || first)) {
-            const int it = maxiter - enq < chunk ? maxiter - enq : chunk;
-            qcd_status s = qcd_cg_iterate(ctx, it);
-            if (s) return s;
+            int it = maxiter - enq < chunk ? maxiter - enq : chunk;
+            if (graph) {
+                // whole graphs only: iterations past maxiter are no-ops (flag 2 is set at k = maxiter)
+                const int reps = (it + GRAPH_ITERS - 1) / GRAPH_ITERS;
+                for (int g = 0; g < reps && result == QCD_OK; ++g) {
+                    if (cudaGraphLaunch(graph, ctx->stream) != cudaSuccess) result = fail(ctx, QCD_ECUDA, "cudaGraphLaunch: %s", cudaGetErrorString(cudaGetLastError()));
+                    ctx->launches += 4 * GRAPH_ITERS;
+                }
+                it = reps * GRAPH_ITERS;
+            } else {
+                result = qcd_cg_iterate(ctx, it);
+            }
+            if (result) break;
             enq += it;
-            CU(ctx, cudaMemcpyAsync(&ctx->h_scal[head * MAXRHS], ctx->d_scal, n * sizeof(CgScalars), cudaMemcpyDeviceToHost, ctx->stream));
-            CU(ctx, cudaEventRecord(ctx->poll_ev[head], ctx->stream));
+            if (cudaMemcpyAsync(&ctx->h_scal[head * MAXRHS], ctx->d_scal, n * sizeof(CgScalars), cudaMemcpyDeviceToHost, ctx->stream) != cudaSuccess ||
+                cudaEventRecord(ctx->poll_ev[head], ctx->stream) != cudaSuccess) {
+                result = fail(ctx, QCD_ECUDA, "qcd_cg: poll copy: %s", cudaGetErrorString(cudaGetLastError()));
+                break;
+            }
             head = (head + 1) % POLL_SLOTS; ++pending; first = false;
             if (chunk < 64) chunk *= 2;
         }
-        CU(ctx, cudaEventSynchronize(ctx->poll_ev[tail]));
+        if (result) break;
+        if (cudaEventSynchronize(ctx->poll_ev[tail]) != cudaSuccess) { result = fail(ctx, QCD_ECUDA, "qcd_cg: %s", cudaGetErrorString(cudaGetLastError())); break; }
         const int state = joint_state(&ctx->h_scal[tail * MAXRHS], n);
         tail = (tail + 1) % POLL_SLOTS; --pending;
         if (state != 0) break;
         if (pending == 0 && enq >= maxiter) break;   // defensive: flag 2 is set when k reaches maxiter
     }
-    return QCD_OK;
+    return result;
 }
 
 extern "C" qcd_status qcd_cg_solve_multi(qcd_ctx *ctx, const qcd_field *U, int n, const qcd_field *const *b, qcd_field *const *x,
@@ -705,7 +752,7 @@ extern "C" qcd_status qcd_cg_solve_multi(qcd_ctx *ctx, const qcd_field *U, int n
     qcd_status s = qcd_cg_begin_multi(ctx, U, n, b, x, m, tol, maxiter);
     if (s) return s;
     s = cg_run(ctx);
-    if (s) { ctx->cg.active = false; return s; }
+    if (s) { const std::string keep = ctx->err; qcd_cg_finish_multi(ctx, nullptr); ctx->err = keep; return s; }
     return qcd_cg_finish_multi(ctx, info);
 }
 

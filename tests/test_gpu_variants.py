@@ -10,6 +10,8 @@ the mixed-precision solver against oracle/variants.py, through the C-ABI, on the
   mixed precision  defect-correction CG vs oracle.variants.mixed_cg: fp64 true residual <= tol
 
 Tolerances as in test_gpu_parity.py (north_star): 1e-13 (fp64), 2e-6 (fp32), per-site measure R10."""
+import contextlib
+
 import numpy as np
 import pytest
 
@@ -377,3 +379,41 @@ def test_mixed_zero_source_and_budget(q):
     info = c64.qcd_cg_solve_mixed(c32, U64, U32, fb, fx, rhs32, e32, 0.1, 1e-10, 1e-3, 10)     # budget of 10 inner iterations
     assert info["status"] == q.QCD_ENOTCONVERGED and not info["converged"] and info["inner_iters"] == 10
     c64.close(); c32.close()
+
+
+# ------------------------------------------------------------------------------------------
+# solver loop on small lattices: CUDA-graph replay
+# ------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("prec", [64, 32])
+def test_cg_graph_replay_matches_plain_loop(q, prec):
+    """On a non-default stream qcd_cg_solve replays a captured graph of 16 iterations; on the legacy
+    default stream it enqueues kernel by kernel.  Same kernels, same order: identical iteration count
+    and bitwise identical solution; both match the oracle."""
+    import torch
+    dims, m = (16, 16, 16, 16), 0.05
+    tol = 1e-10 if prec == 64 else 1e-5
+    U = qcd_inputs.gauge_field(dims, "near_identity", seed=0, eps=0.3)
+    b = qcd_inputs.gaussian_source(dims, seed=1)
+    res = []
+    for use_stream in (False, True):
+        stream = torch.cuda.Stream() if use_stream else None
+        with (torch.cuda.stream(stream) if use_stream else contextlib.nullcontext()):
+            ctx = q.Context(dims, prec, stream=stream)
+            fU = ctx.field(q.QCD_GAUGE).upload(U)
+            fb = ctx.field(q.QCD_SPINOR_EVEN).upload(b)
+            fx = ctx.field(q.QCD_SPINOR_EVEN)
+            n0 = ctx.qcd_launch_count()
+            info = ctx.qcd_cg_solve(fU, fb, fx, m, tol, 10000)
+            launches = ctx.qcd_launch_count() - n0
+            res.append((info, fx.download(), launches))
+            # maxiter that is not a multiple of the graph length: stops exactly there
+            info2 = ctx.qcd_cg_solve(fU, fb, fx, m, 1e-300, 37)
+            assert info2["iters"] == 37 and not info2["converged"] and info2["status"] == q.QCD_ENOTCONVERGED
+            ctx.close()
+    (i0, x0, l0), (i1, x1, l1) = res
+    assert i0["converged"] and i1["converged"] and i0["iters"] == i1["iters"]
+    assert np.array_equal(x0, x1)
+    assert l1 >= 4 * i1["iters"] and l0 >= 4 * i0["iters"]
+    _, oinfo = oracle.cg(dims, _rounded(U, prec).astype(x0.dtype), _rounded(b, prec).astype(x0.dtype), m, tol, 10000)
+    assert iters_close(i1["iters"], oinfo["iters"])
+    assert oracle.true_residual(dims, _rounded(U, prec), _rounded(b, prec), x1.astype(np.complex128), m) <= tol * (1.0 if prec == 64 else 1.5)
