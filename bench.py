@@ -66,6 +66,8 @@ def parse_args():
     ap.add_argument("--prec", type=int, default=64, choices=(64, 32), help="precision of --variants-only")
     ap.add_argument("--nmulti", default="1,2,3,4,6,8", help="NMULTI values of --variants-only")
     ap.add_argument("--reps", type=int, default=10, help="timed launches per variant of --variants-only")
+    ap.add_argument("--kernel", type=int, default=0,
+                    help="qcd_set_dslash_variant for --variants-only (0 default choice, 4 staged kernel, 5 register kernel)")
     return ap.parse_args()
 
 
@@ -567,6 +569,7 @@ def run_variants_only(args):
     _, U, _ = make_inputs(dims)
     ctx = q.Context(dims, args.prec)
     fU = ctx.field(q.QCD_GAUGE).upload(U)
+    ctx.qcd_set_dslash_variant(args.kernel)
     rows = variants_sweep(q, torch, ctx, fU, dims, peak, tuple(int(v) for v in args.nmulti.split(",")), args.reps)
     print(json.dumps({"variants": rows, "lattice": list(dims), "prec": args.prec, "gpu_launches": ctx.qcd_launch_count()}), flush=True)
     ctx.close()

@@ -218,6 +218,15 @@ long long qcd_launch_count(const qcd_ctx *ctx);
  *   variant 0 = default.  Unknown variants -> QCD_EINVAL.
  */
 qcd_status qcd_set_dslash_variant(qcd_ctx *ctx, int variant);
+/*
+ * Traversal order of the Dslash threads: the sites are walked in
+ * chunks of `width` rows of x2 ((x0,x1) fastest, x2 inside the chunk, then x3, then the chunk),
+ * which keeps the time-neighbour spinors of several vectors inside the L2.  A pure permutation of
+ * the work: results are independent of it.  width = 0: chosen by the library from the lattice,
+ * the precision and the number of vectors (N2, i.e. the plain order, for one vector up to 64^4);
+ * otherwise a divisor of N2.  Else QCD_EINVAL.
+ */
+qcd_status qcd_set_traversal_chunk(qcd_ctx *ctx, int width);
 
 /* Re<a,b> over a half-field pair of the same kind (deterministic two-stage reduction,
  * double accumulation); synchronises.  Used by tests and by callers that need norms. */

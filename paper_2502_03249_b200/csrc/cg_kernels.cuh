@@ -55,7 +55,7 @@ struct RhsPtrs {
 
 template <typename T>
 __global__ void __launch_bounds__(BLAS_BLOCK) cg_init_kernel(
-    int n16, const RhsPtrs<typename Vec16<T>::type> ptrs,
+    int n16, const __grid_constant__ RhsPtrs<typename Vec16<T>::type> ptrs,
     typename Vec16<T>::type *__restrict__ r, typename Vec16<T>::type *__restrict__ p,
     double tol, int maxiter, double *partials, CgScalars *scal)
 {
@@ -101,7 +101,7 @@ __global__ void __launch_bounds__(BLAS_BLOCK) cg_init_kernel(
 
 template <typename T>
 __global__ void __launch_bounds__(BLAS_BLOCK) cg_update_xr_kernel(
-    int n16, const RhsPtrs<typename Vec16<T>::type> ptrs, typename Vec16<T>::type *__restrict__ r,
+    int n16, const __grid_constant__ RhsPtrs<typename Vec16<T>::type> ptrs, typename Vec16<T>::type *__restrict__ r,
     const typename Vec16<T>::type *__restrict__ p, const typename Vec16<T>::type *__restrict__ Ap,
     double *partials, CgScalars *scal)
 {

@@ -104,13 +104,25 @@ __device__ __forceinline__ void load_link(C u[9], const C *p, size_t Vh, uint64_
     for (int k = 0; k < 3 * NROW; ++k) u[k] = ld_stream(p + (size_t)k * Vh, pol);
 }
 
+// x -> sign * x for sign = +-1, as a flip of the IEEE sign bit: exact, and an integer-pipe
+// operation (the fp64 pipe is the scarce one once several vectors share a link).
+__device__ __forceinline__ double flip_sign(double x, unsigned neg)
+{
+    return __hiloint2double(__double2hiint(x) ^ (int)(neg << 31), __double2loint(x));
+}
+__device__ __forceinline__ float flip_sign(float x, unsigned neg)
+{
+    return __int_as_float(__float_as_int(x) ^ (int)(neg << 31));
+}
+
 template <typename T, typename C>
 __device__ __forceinline__ void load_spinor(C p[3], const C *f, size_t Vh, int site, T sign, uint64_t pol)
 {
 #pragma unroll
     for (int c = 0; c < 3; ++c) p[c] = ld_keep(f + (size_t)c * Vh + site, pol);
+    const unsigned neg = sign < (T)0 ? 1u : 0u;
 #pragma unroll
-    for (int c = 0; c < 3; ++c) { p[c].x *= sign; p[c].y *= sign; }     // exact: sign is +-1
+    for (int c = 0; c < 3; ++c) { p[c].x = flip_sign(p[c].x, neg); p[c].y = flip_sign(p[c].y, neg); }
 }
 
 template <typename C>
@@ -118,6 +130,56 @@ __device__ __forceinline__ void vec_acc(C acc[3], const C p[3])
 {
 #pragma unroll
     for (int c = 0; c < 3; ++c) { acc[c].x += p[c].x; acc[c].y += p[c].y; }
+}
+
+// out = acc (MODE 0) or m^2 v - acc (MODE >= 1); MODE 2 also accumulates Re<v,out> per vector.
+template <typename T, int MODE, int NRHS>
+__device__ __forceinline__ void dslash_epilogue(const DslashArgs<T, NRHS> &a, int cb, typename Cplx<T>::type (&acc)[NRHS][3],
+                                                double (&dot)[NRHS])
+{
+    typedef typename Cplx<T>::type C;
+    const size_t Vh = (size_t)a.L.Vh;
+#pragma unroll
+    for (int r = 0; r < NRHS; ++r) {
+        if (MODE >= 1) {
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+                const C vv = a.v[r][(size_t)c * Vh + cb];
+                C o;
+                o.x = fma(a.m2, vv.x, -acc[r][c].x);
+                o.y = fma(a.m2, vv.y, -acc[r][c].y);
+                a.out[r][(size_t)c * Vh + cb] = o;
+                if (MODE == 2) dot[r] += (double)vv.x * (double)o.x + (double)vv.y * (double)o.y;
+            }
+        } else {
+#pragma unroll
+            for (int c = 0; c < 3; ++c) a.out[r][(size_t)c * Vh + cb] = acc[r][c];
+        }
+    }
+}
+
+// MODE 2: two-stage reduction of the per-vector Re<p,Mp> and the CG alpha step in the last block.
+template <typename T, int MODE, int NRHS, int BLOCK>
+__device__ __forceinline__ void dslash_reduce(const DslashArgs<T, NRHS> &a, double (&dot)[NRHS])
+{
+    if (MODE == 2) {
+        __shared__ double smem[NRHS * (BLOCK / 32)];
+        __shared__ int last;
+        if (publish_partials<BLOCK, NRHS>(dot, a.partials, (size_t)gridDim.x, &a.scal[0].ticket, smem, &last)) {
+            for (int r = 0; r < NRHS; ++r) {
+                const double pAp = final_sum<BLOCK>(a.partials + (size_t)r * gridDim.x, (int)gridDim.x, smem);
+                if (threadIdx.x == 0) {
+                    CgScalars *s = a.scal + r;
+                    if (s->flag == 0) {
+                        s->pAp = pAp;
+                        if (!(pAp > 0.0)) s->flag = 3;          // breakdown: <p,Mp> <= 0 or NaN
+                        else s->alpha = s->rr / pAp;
+                    }
+                }
+                __syncthreads();
+            }
+        }
+    }
 }
 
 template <typename T, int MODE, int NROW, int TG, int NRHS, int BLOCK, int MINB>
@@ -131,8 +193,9 @@ __global__ void __launch_bounds__(BLOCK, MINB) dslash_kernel(const DslashArgs<T,
         if (all_done) return;
     }
 
-    const int cb = blockIdx.x * BLOCK + threadIdx.x;
-    const bool active = cb < a.L.Vh;
+    const int tid = blockIdx.x * BLOCK + threadIdx.x;
+    const bool active = tid < a.L.Vh;
+    const int cb = active ? traversal_site(a.L, tid) : tid;
     const size_t Vh = (size_t)a.L.Vh;
     double dot[NRHS];
 #pragma unroll
@@ -207,43 +270,117 @@ __global__ void __launch_bounds__(BLOCK, MINB) dslash_kernel(const DslashArgs<T,
             }
         }
 
+        dslash_epilogue<T, MODE, NRHS>(a, cb, acc, dot);
+    }
+    dslash_reduce<T, MODE, NRHS, BLOCK>(a, dot);
+}
+
+// ------------------------------------------------------------------------------------------
+// Staged variant for several vectors (NRHS >= 3).  With 6 NRHS accumulators per thread the
+// register file allows only 8 warps per SM, and a warp that waits for a link from DRAM has
+// nothing else to issue: the kernel above is latency-bound there (ncu: 70 % long-scoreboard
+// stalls, no memory unit above 45 %).  Here every thread copies its own links with cp.async
+// into its own column of shared memory -- DEPTH hops ahead, without holding registers -- and
+// reads a link back (conflict-free LDS.128) only when the hop is computed.  No thread reads
+// another thread's column, so no block-level barrier is needed: cp.async.wait_group orders a
+// thread's copies with its own reads.  Hop h = 2 mu + (0: forward, 1: backward); ring of DEPTH
+// hops: after hop h is consumed its column is refilled with hop h + DEPTH.
+// ------------------------------------------------------------------------------------------
+template <typename T, int MODE, int NROW, int TG, int NRHS, int BLOCK, int MINB, int DEPTH>
+__global__ void __launch_bounds__(BLOCK, MINB) dslash_staged_kernel(const DslashArgs<T, NRHS> a)
+{
+    typedef typename Cplx<T>::type C;
+    extern __shared__ __align__(16) unsigned char staged_smem[];
+    C (*ring)[BLOCK] = reinterpret_cast<C (*)[BLOCK]>(staged_smem);       // [DEPTH * 3 NROW][BLOCK]
+    if (a.check_flag) {
+        bool all_done = true;
 #pragma unroll
-        for (int r = 0; r < NRHS; ++r) {
-            if (MODE >= 1) {
+        for (int r = 0; r < NRHS; ++r) all_done = all_done && (a.scal[r].flag != 0);
+        if (all_done) return;
+    }
+
+    const int tid = blockIdx.x * BLOCK + threadIdx.x;
+    const bool active = tid < a.L.Vh;
+    const int cb = active ? traversal_site(a.L, tid) : tid;
+    const size_t Vh = (size_t)a.L.Vh;
+    double dot[NRHS];
 #pragma unroll
-                for (int c = 0; c < 3; ++c) {
-                    const C vv = a.v[r][(size_t)c * Vh + cb];
-                    C o;
-                    o.x = fma(a.m2, vv.x, -acc[r][c].x);
-                    o.y = fma(a.m2, vv.y, -acc[r][c].y);
-                    a.out[r][(size_t)c * Vh + cb] = o;
-                    if (MODE == 2) dot[r] += (double)vv.x * (double)o.x + (double)vv.y * (double)o.y;
+    for (int r = 0; r < NRHS; ++r) dot[r] = 0.0;
+
+    if (active) {
+        const SiteGeom g = site_geometry(a.L, a.parity, cb);
+        const uint64_t pol_stream = l2_policy_evict_first();
+        const uint64_t pol_keep = l2_policy_evict_last();
+        const C *Uf = a.U + (size_t)(a.parity * 12 * NROW) * Vh + cb;
+        const C *Ub = a.U + (size_t)((1 - a.parity) * 12 * NROW) * Vh;
+
+        // issue the copies of hop h into ring column h % DEPTH (an empty group for a unit link)
+        auto issue = [&](int h) {
+            const int mu = h >> 1;
+            const bool fwd = (h & 1) == 0;
+            const bool unit = TG && mu == 3 && (fwd ? g.x3 != 0 : g.x3 != 1);
+            const C *src = fwd ? Uf + (size_t)(mu * 3 * NROW) * Vh : Ub + (size_t)(mu * 3 * NROW) * Vh + g.nb[mu];
+            if (!unit) {
+#pragma unroll
+                for (int k = 0; k < 3 * NROW; ++k)
+                    cp_async_stream(&ring[(h % DEPTH) * 3 * NROW + k][threadIdx.x], src + (size_t)k * Vh, pol_stream);
+            }
+            cp_async_commit();
+        };
+#pragma unroll
+        for (int h = 0; h < DEPTH; ++h) issue(h);
+
+        C acc[NRHS][3];
+#pragma unroll
+        for (int r = 0; r < NRHS; ++r)
+            acc[r][0].x = acc[r][0].y = acc[r][1].x = acc[r][1].y = acc[r][2].x = acc[r][2].y = (T)0;
+
+        // the neighbour vectors of hop h + 1 are requested before hop h is computed when the
+        // registers allow a second set (PIPE), so an L2 round trip hides behind 36 NRHS FMAs
+        constexpr bool PIPE = (sizeof(T) == 8 ? NRHS <= 4 : NRHS <= 8);
+        auto hop_site = [&](int h) { return (h & 1) == 0 ? g.nf[h >> 1] : g.nb[h >> 1]; };
+        auto hop_sign = [&](int h) { return (T)((h & 1) == 0 ? g.sf[h >> 1] : g.sb[h >> 1]); };
+        C pbuf[PIPE ? 2 : 1][NRHS][3];
+        if (PIPE) {
+#pragma unroll
+            for (int r = 0; r < NRHS; ++r) load_spinor<T, C>(pbuf[0][r], a.in[r], Vh, hop_site(0), hop_sign(0), pol_keep);
+        }
+#pragma unroll
+        for (int h = 0; h < 8; ++h) {
+            const int mu = h >> 1;
+            const bool fwd = (h & 1) == 0;
+            const bool unit = TG && mu == 3 && (fwd ? g.x3 != 0 : g.x3 != 1);
+            C (&p)[NRHS][3] = pbuf[PIPE ? (h & 1) : 0];
+            if (PIPE) {
+                if (h + 1 < 8) {
+#pragma unroll
+                    for (int r = 0; r < NRHS; ++r)
+                        load_spinor<T, C>(pbuf[(h + 1) & 1][r], a.in[r], Vh, hop_site(h + 1), hop_sign(h + 1), pol_keep);
                 }
             } else {
 #pragma unroll
-                for (int c = 0; c < 3; ++c) a.out[r][(size_t)c * Vh + cb] = acc[r][c];
+                for (int r = 0; r < NRHS; ++r) load_spinor<T, C>(p[r], a.in[r], Vh, hop_site(h), hop_sign(h), pol_keep);
             }
-        }
-    }
-
-    if (MODE == 2) {
-        __shared__ double smem[NRHS * (BLOCK / 32)];
-        __shared__ int last;
-        if (publish_partials<BLOCK, NRHS>(dot, a.partials, (size_t)gridDim.x, &a.scal[0].ticket, smem, &last)) {
-            for (int r = 0; r < NRHS; ++r) {
-                const double pAp = final_sum<BLOCK>(a.partials + (size_t)r * gridDim.x, (int)gridDim.x, smem);
-                if (threadIdx.x == 0) {
-                    CgScalars *s = a.scal + r;
-                    if (s->flag == 0) {
-                        s->pAp = pAp;
-                        if (!(pAp > 0.0)) s->flag = 3;          // breakdown: <p,Mp> <= 0 or NaN
-                        else s->alpha = s->rr / pAp;
-                    }
+            // groups committed so far: min(8, h + DEPTH); hop h needs groups 0 .. h complete
+            cp_async_wait((h + DEPTH < 8 ? h + DEPTH : 8) - h - 1);
+            if (!unit) {
+                C u[9];
+#pragma unroll
+                for (int k = 0; k < 3 * NROW; ++k) u[k] = ring[(h % DEPTH) * 3 * NROW + k][threadIdx.x];
+                if (NROW == 2) reconstruct_third_row<C>(u);
+#pragma unroll
+                for (int r = 0; r < NRHS; ++r) {
+                    if (fwd) mat_vec_acc<T, C>(acc[r], u, p[r]); else matdag_vec_acc<T, C>(acc[r], u, p[r]);
                 }
-                __syncthreads();
+            } else {
+#pragma unroll
+                for (int r = 0; r < NRHS; ++r) vec_acc<C>(acc[r], p[r]);
             }
+            if (h + DEPTH < 8) issue(h + DEPTH);
         }
+        dslash_epilogue<T, MODE, NRHS>(a, cb, acc, dot);
     }
+    dslash_reduce<T, MODE, NRHS, BLOCK>(a, dot);
 }
 
 } // namespace qcd

@@ -39,9 +39,42 @@ static cudaError_t launch_cfg(const DslashLaunch &d)
     return cudaGetLastError();
 }
 
+// Staged kernel (links through shared memory by cp.async, dslash.cuh): ring of STAGE_DEPTH hops.
+enum { STAGE_DEPTH = 4 };
+template <typename T, int NRHS> struct StagedCfg { enum { BLOCK = 128, MINB = sizeof(T) == 8 ? (NRHS <= 4 ? 3 : 2) : (NRHS <= 4 ? 4 : 3) }; };
+
+template <typename T, int MODE, int NROW, int TG, int NRHS>
+static cudaError_t launch_staged(const DslashLaunch &d)
+{
+    typedef typename Cplx<T>::type C;
+    enum { BLOCK = StagedCfg<T, NRHS>::BLOCK, MINB = StagedCfg<T, NRHS>::MINB };
+    const size_t smem = (size_t)STAGE_DEPTH * 3 * NROW * BLOCK * sizeof(C);
+    auto kernel = dslash_staged_kernel<T, MODE, NROW, TG, NRHS, BLOCK, MINB, STAGE_DEPTH>;
+    static bool configured = false;          // one flag per instantiation
+    if (!configured) {
+        const cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        configured = true;
+    }
+    DslashArgs<T, NRHS> a;
+    a.L = d.L; a.parity = d.parity; a.U = (const C *)d.U;
+    for (int r = 0; r < NRHS; ++r) { a.in[r] = (const C *)d.in[r]; a.out[r] = (C *)d.out[r]; a.v[r] = (const C *)d.v[r]; }
+    a.m2 = (T)d.m2; a.partials = d.partials; a.scal = d.scal; a.check_flag = d.check_flag;
+    const int grid = (d.L.Vh + BLOCK - 1) / BLOCK;
+    kernel<<<grid, BLOCK, smem, d.stream>>>(a);
+    return cudaGetLastError();
+}
+
 template <typename T, int MODE, int NROW, int TG, int NRHS>
 static cudaError_t launch_nrhs(const DslashLaunch &d)
 {
+    // variant 4 forces the staged kernel, variant 5 the register kernel (A/B sweeps); otherwise the
+    // staged kernel serves the (precision, NRHS, link rows) where it measured faster at 64^4
+    // (profiles/README.md "staged vs register kernel"): fp64 n = 3, 4; fp32 n = 8, and n >= 4 on two-row links
+    if constexpr (MODE != 1) {
+        constexpr bool staged_wins = sizeof(T) == 8 ? (NRHS == 3 || NRHS == 4) : (NRHS == 8 || (NROW == 2 && NRHS >= 4));
+        if (d.variant == 4 || (d.variant != 5 && staged_wins)) return launch_staged<T, MODE, NROW, TG, NRHS>(d);
+    }
     if constexpr (NRHS == 1 && TG == 0) {
         switch (d.variant) {       // block-shape sweep of the headline kernel
         case 1: return launch_cfg<T, MODE, NROW, TG, 1, 64, 8>(d);

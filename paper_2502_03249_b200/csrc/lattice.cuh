@@ -16,6 +16,7 @@ struct Lattice {
     int s1;       // cb stride of x1 (= h)
     int s2;       // cb stride of x2 (= h N1)
     int s3;       // cb stride of x3 (= h N1 N2)
+    int W;        // traversal chunk width in x2 (divides N2; N2 = plain cb order), see traversal_site
 };
 
 template <typename T> struct Cplx;
@@ -80,6 +81,55 @@ __device__ __forceinline__ float4 ld_keep(const float4 *p, uint64_t pol)
     asm volatile("ld.global.nc.L2::cache_hint.v4.f32 {%0,%1,%2,%3}, [%4], %5;"
                  : "=f"(r.x), "=f"(r.y), "=f"(r.z), "=f"(r.w) : "l"(p), "l"(pol));
     return r;
+}
+
+// Asynchronous global -> shared copies (LDGSTS): the data never passes through registers, so a
+// thread can keep many link loads in flight without holding registers for them.  16-byte copies
+// bypass L1 (.cg); 8-byte copies exist only as .ca.  L2 policy operand as for ld_stream.
+__device__ __forceinline__ void cp_async_stream(double2 *smem_dst, const double2 *src, uint64_t pol)
+{
+    const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
+    asm volatile("cp.async.cg.shared.global.L2::cache_hint [%0], [%1], 16, %2;" :: "r"(d), "l"(src), "l"(pol) : "memory");
+}
+__device__ __forceinline__ void cp_async_stream(float2 *smem_dst, const float2 *src, uint64_t pol)
+{
+    const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
+    asm volatile("cp.async.ca.shared.global.L2::cache_hint [%0], [%1], 8, %2;" :: "r"(d), "l"(src), "l"(pol) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+// wait until at most `pending` of this thread's most recent groups are still in flight
+// (the operand must be an immediate: the switch folds once the caller's loop is unrolled)
+__device__ __forceinline__ void cp_async_wait(int pending)
+{
+    switch (pending) {
+    case 0: asm volatile("cp.async.wait_group 0;" ::: "memory"); break;
+    case 1: asm volatile("cp.async.wait_group 1;" ::: "memory"); break;
+    case 2: asm volatile("cp.async.wait_group 2;" ::: "memory"); break;
+    case 3: asm volatile("cp.async.wait_group 3;" ::: "memory"); break;
+    case 4: asm volatile("cp.async.wait_group 4;" ::: "memory"); break;
+    case 5: asm volatile("cp.async.wait_group 5;" ::: "memory"); break;
+    case 6: asm volatile("cp.async.wait_group 6;" ::: "memory"); break;
+    default: asm volatile("cp.async.wait_group 7;" ::: "memory"); break;
+    }
+}
+
+// Traversal order of the Dslash threads.  Thread t of the grid handles site cb = t in the plain
+// order.  With several vectors per link load the spinor working set between the two uses of a
+// time-neighbour (two full time slices) outgrows the L2, and every spinor is fetched from DRAM
+// more than once.  The chunked order walks x2 in chunks of W rows: (x0, x1) fastest, then x2
+// inside the chunk, then x3, then the chunk -- the x3 reuse distance shrinks from 2 N2 to 2 W
+// rows of h N1 sites, at the price of re-reading 2 of every W rows at the chunk edges.
+// A pure permutation of which thread handles which site: results do not depend on it.
+__device__ __forceinline__ int traversal_site(const Lattice &L, int t)
+{
+    if (L.W == L.N2) return t;
+    const unsigned R = (unsigned)L.s2;                     // sites per x2-row
+    const unsigned rowp = (unsigned)t / R, off = (unsigned)t - rowp * R;
+    const unsigned per = (unsigned)(L.W * L.N3);           // rows per chunk
+    const unsigned chunk = rowp / per, rem = rowp - chunk * per;
+    const unsigned x3 = rem / (unsigned)L.W, x2lo = rem - x3 * (unsigned)L.W;
+    const unsigned row = chunk * (unsigned)L.W + x2lo + (unsigned)L.N2 * x3;
+    return (int)(row * R + off);
 }
 
 // Site geometry of one checkerboard index: coordinates, the 8

@@ -65,6 +65,7 @@ struct qcd_ctx {
     size_t ws_bytes;
     CgState cg;
     int variant;
+    int chunk;                // Dslash traversal chunk width in x2: 0 = automatic, else a divisor of N2
     long long launches;
     // profiling
     bool prof_on;
@@ -165,7 +166,8 @@ extern "C" qcd_status qcd_init(qcd_ctx **out, const int dims[4], int precision, 
     c->L.s1 = c->L.h; c->L.s2 = c->L.h * dims[1]; c->L.s3 = c->L.h * dims[1] * dims[2];
     c->prec = precision; c->rsize = precision == 64 ? 8 : 4;
     c->stream = (cudaStream_t)cuda_stream;
-    c->variant = 0; c->launches = 0;
+    c->variant = 0; c->launches = 0; c->chunk = 0;
+    c->L.W = dims[2];
     c->prof_on = false; c->prof_created = false; c->prof_n = c->prof_dropped = 0;
     c->ws = nullptr; c->ws_bytes = 0;
     memset(&c->cg, 0, sizeof c->cg);
@@ -302,10 +304,18 @@ extern "C" qcd_status qcd_profile_read(qcd_ctx *ctx, int which, int *launches, d
 
 extern "C" long long qcd_launch_count(const qcd_ctx *ctx) { return ctx ? ctx->launches : 0; }
 
+extern "C" qcd_status qcd_set_traversal_chunk(qcd_ctx *ctx, int width)
+{
+    if (!ctx) return QCD_EINVAL;
+    if (width < 0 || (width > 0 && ctx->L.N2 % width)) return fail(ctx, QCD_EINVAL, "qcd_set_traversal_chunk: width must be 0 (automatic) or a divisor of N2");
+    ctx->chunk = width;
+    return QCD_OK;
+}
+
 extern "C" qcd_status qcd_set_dslash_variant(qcd_ctx *ctx, int variant)
 {
     if (!ctx) return QCD_EINVAL;
-    if (variant < 0 || variant > 3) return fail(ctx, QCD_EINVAL, "qcd_set_dslash_variant: unknown variant");
+    if (variant < 0 || variant > 5) return fail(ctx, QCD_EINVAL, "qcd_set_dslash_variant: unknown variant");
     ctx->variant = variant;
     return QCD_OK;
 }
@@ -374,13 +384,31 @@ extern "C" qcd_status qcd_field_download(const qcd_field *f, void *host)
 // ------------------------------------------------------------------------------------------
 // Dslash launches
 // ------------------------------------------------------------------------------------------
+// Chunk width of the traversal (lattice.cuh traversal_site): the largest divisor W of N2 for which
+// four slabs (three time slices of inputs in flight plus the outputs being written) of W rows of n
+// vectors fit a fixed share of the L2.  One vector at 64^4 gives W = N2 (plain order).
+enum { CHUNK_BUDGET_BYTES = 32 << 20 };
+static int traversal_chunk(const qcd_ctx *c, int n)
+{
+    const int N2 = c->L.N2;
+    if (c->chunk > 0) return c->chunk;
+    const double row_bytes = (double)c->L.s2 * 6.0 * c->rsize * n;
+    int W = N2;
+    while (W > 1 && 4.0 * row_bytes * W > (double)CHUNK_BUDGET_BYTES) {
+        int next = W - 1;
+        while (next > 1 && N2 % next) --next;
+        W = next;
+    }
+    return W;
+}
+
 // out[r](parity) = D in[r](1-parity), r < n; mode >= 1 adds the M epilogue with v[r] (parity of out)
 static qcd_status dslash_launch(qcd_ctx *c, int mode, const qcd_field *U, int n, void *const *out, const void *const *in,
                                 int parity, const void *const *v, double m, CgScalars *scal, int check_flag)
 {
     DslashLaunch d;
     d.mode = mode; d.tg = U->tg; d.nrhs = n; d.variant = c->variant;
-    d.L = c->L; d.parity = parity; d.U = U->ptr;
+    d.L = c->L; d.L.W = traversal_chunk(c, n); d.parity = parity; d.U = U->ptr;
     for (int r = 0; r < MAXRHS; ++r) {
         d.in[r] = r < n ? in[r] : nullptr;
         d.out[r] = r < n ? out[r] : nullptr;
