@@ -99,9 +99,7 @@ def test_dslash_full_size(q, config, prec):
     fo = ctx.field(q.QCD_SPINOR_ODD)
     fe2 = ctx.field(q.QCD_SPINOR_EVEN)
     ctx.qcd_dslash_oe(fU, fo, fe)              # t = D_oe b
-    ctx.qcd_dslash_eo(fU, fe2, fo)             # D_eo t
     got_o = fo.download()
-    got_e = fe2.download()
     Ur, br = rounded(U, prec), rounded(b, prec)
     tol = DSLASH_TOL[prec]
     R_o = np.sqrt(np.mean(np.linalg.norm(got_o[1::2], axis=1) ** 2))      # rms site norm scale (R10)
@@ -112,8 +110,17 @@ def test_dslash_full_size(q, config, prec):
         d = np.linalg.norm(got_o[lex(dims, x)] - ref) / max(np.linalg.norm(ref), 0.1 * R_o)
         worst = max(worst, d)
     assert worst <= tol, worst
-    # second hop: the oracle is applied to what the device holds for t (already in device precision)
-    t_in = got_o.astype(np.complex128)
+    # whole field, element by element
+    par = qcd_inputs.site_parity(dims)
+    ref_o = oracle.dslash(dims, Ur, br, 1)
+    assert dslash_rel_err(got_o[par == 1], ref_o[par == 1]) <= tol
+    assert not got_o[par == 0].any()
+    # second hop (D_eo): device and oracle both start from the ORACLE's t, rounded to the device precision
+    t_in = rounded(ref_o, prec)
+    del ref_o
+    fo.upload(t_in)
+    ctx.qcd_dslash_eo(fU, fe2, fo)
+    got_e = fe2.download()
     R_e = np.sqrt(np.mean(np.linalg.norm(got_e[::2], axis=1) ** 2))
     worst = 0.0
     for x in sample_sites(dims, 0, 300, seed=100 + config):
@@ -121,15 +128,70 @@ def test_dslash_full_size(q, config, prec):
         d = np.linalg.norm(got_e[lex(dims, x)] - ref) / max(np.linalg.norm(ref), 0.1 * R_e)
         worst = max(worst, d)
     assert worst <= tol, worst
-    # whole field, element by element
-    par = qcd_inputs.site_parity(dims)
-    ref_o = oracle.dslash(dims, Ur, br, 1)
-    assert dslash_rel_err(got_o[par == 1], ref_o[par == 1]) <= tol
-    assert not got_o[par == 0].any()
-    del ref_o
     ref_e = oracle.dslash(dims, Ur, t_in, 0)
     assert dslash_rel_err(got_e[par == 0], ref_e[par == 0]) <= tol
     assert V == par.size
+    ctx.close()
+
+
+# ------------------------------------------------------------------------------------------
+# the paper's variants at full size, as bench.py launches them
+# ------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("n", [4, 8])
+def test_multi_vector_two_row_64(q, n):
+    """configs[4], fp64, two-row links compressed on the device, n vectors per link load: at this size
+    the library chunks the traversal (W < N2) and picks the staged kernel for n = 4, the register
+    kernel for n = 8 -- exactly what bench.py's variants sweep times.  Sampled sites, literal Eq. (1)."""
+    cfg, U, b = inputs(4)
+    dims = cfg["dims"]
+    ctx = q.Context(dims, 64)
+    fU = ctx.field(q.QCD_GAUGE).upload(U)
+    f12 = ctx.field(q.QCD_GAUGE_2ROW)
+    ctx.qcd_gauge_compress(fU, f12)
+    fU.free()
+    srcs = [b] + [qcd_inputs.gaussian_source(dims, seed=40 + i) for i in range(1, n)]
+    fin = [ctx.field(q.QCD_SPINOR_EVEN).upload(s_) for s_ in srcs]
+    fout = [ctx.field(q.QCD_SPINOR_ODD) for _ in range(n)]
+    ctx.qcd_dslash_oe_multi(f12, fout, fin)
+    sites = sample_sites(dims, 1, 60, seed=7)
+    for i in range(n):
+        got = fout[i].download()
+        R = np.sqrt(np.mean(np.linalg.norm(got[1::2], axis=1) ** 2))
+        worst = 0.0
+        for x in sites:
+            ref = oracle.dslash_site(dims, U, srcs[i], x)       # fp64: the rebuilt third row is the third row (1e-15)
+            worst = max(worst, np.linalg.norm(got[lex(dims, x)] - ref) / max(np.linalg.norm(ref), 0.1 * R))
+        assert worst <= DSLASH_TOL[64], (i, worst)
+        del got
+    ctx.close()
+
+
+@pytest.mark.parametrize("prec", [64, 32])
+def test_temporal_gauge_two_row_32(q, prec):
+    """configs[2] (the paper's Table 2 lattice): links fixed to temporal gauge by the ORACLE, rounded,
+    uploaded as two-row links and marked; n = 1 and n = 4; whole fields against the oracle."""
+    import oracle.variants as ov
+    cfg, U, b = inputs(2)
+    dims = cfg["dims"]
+    Ufix, g = ov.temporal_gauge(dims, U)
+    x3 = qcd_inputs.site_coords(dims)[:, 3]
+    Ufix[x3 != 0, 3] = np.eye(3)
+    Uref = ov.reconstruct12(ov.compress12(rounded(Ufix, prec)))
+    srcs = [ov.rotate_spinor(g, b)] + [qcd_inputs.gaussian_source(dims, seed=50 + i) for i in range(1, 4)]
+    par = qcd_inputs.site_parity(dims)
+    ctx = q.Context(dims, prec)
+    f12 = ctx.field(q.QCD_GAUGE_2ROW).upload(Ufix)
+    ctx.qcd_gauge_set_temporal_unit(f12, True)
+    fin = [ctx.field(q.QCD_SPINOR_EVEN).upload(s_) for s_ in srcs]
+    fout = [ctx.field(q.QCD_SPINOR_ODD) for _ in srcs]
+    refs = [oracle.dslash(dims, Uref, rounded(s_, prec), 1) for s_ in srcs]
+    ctx.qcd_dslash_oe(f12, fout[0], fin[0])
+    assert dslash_rel_err(fout[0].download()[par == 1], refs[0][par == 1]) <= DSLASH_TOL[prec]
+    for f in fout:
+        f.buf.zero_()
+    ctx.qcd_dslash_oe_multi(f12, fout, fin)
+    for i in range(4):
+        assert dslash_rel_err(fout[i].download()[par == 1], refs[i][par == 1]) <= DSLASH_TOL[prec], i
     ctx.close()
 
 
