@@ -288,28 +288,35 @@ def cg_multi_report(q, torch, device, dims, prec, fU_full, m, ns=(1, 2, 4), iter
 
 
 def small_lattice_report(q, torch, device):
-    """configs[1] (16^4, links fit the L2): the solve is launch- and reduction-latency bound (PAPER.md:54);
-    kernel-by-kernel enqueue on the default stream vs CUDA-graph replay of 16 iterations on a side stream."""
-    import contextlib
+    """configs[1] (16^4, links fit the L2): the solve is launch- and reduction-latency bound.
+    The three solver loops of qcd_set_cg_loop: kernel-by-kernel enqueue, CUDA-graph replay of 16 iterations
+    (side stream), and the persistent cooperative kernel (the library's choice at this size)."""
     dims = (16, 16, 16, 16)
     cfg, U, b = make_inputs(dims, 1)
     rows = []
-    for name, side in (("kernel-by-kernel enqueue (default stream)", False), ("CUDA-graph replay, 16 iterations per launch (side stream)", True)):
-        stream = torch.cuda.Stream(device=device) if side else None
-        with (torch.cuda.stream(stream) if side else contextlib.nullcontext()):
-            for prec, tol in ((64, cfg["tol64"]), (32, cfg["tol32"])):
-                ctx = q.Context(dims, prec, stream=stream, device=device)
-                fU = ctx.field(q.QCD_GAUGE).upload(U)
-                fb = ctx.field(q.QCD_SPINOR_EVEN).upload(b)
-                fx = ctx.field(q.QCD_SPINOR_EVEN)
+    stream = torch.cuda.Stream(device=device)
+    with torch.cuda.stream(stream):
+        for prec, tol in ((64, cfg["tol64"]), (32, cfg["tol32"])):
+            ctx = q.Context(dims, prec, stream=stream, device=device)
+            fU = ctx.field(q.QCD_GAUGE).upload(U)
+            fb = ctx.field(q.QCD_SPINOR_EVEN).upload(b)
+            fx = ctx.field(q.QCD_SPINOR_EVEN)
+            for loop, name in ((1, "kernel-by-kernel enqueue"), (2, "CUDA-graph replay, 16 iterations per launch"),
+                               (3, "persistent cooperative kernel (one launch per solve)")):
+                ctx.qcd_set_cg_loop(loop)
                 ctx.qcd_cg_solve(fU, fb, fx, cfg["m"], tol, cfg["maxiter"])
-                t0 = time.perf_counter()
-                info = ctx.qcd_cg_solve(fU, fb, fx, cfg["m"], tol, cfg["maxiter"])
-                wall = time.perf_counter() - t0
+                best = None
+                for _ in range(3):
+                    t0 = time.perf_counter()
+                    info = ctx.qcd_cg_solve(fU, fb, fx, cfg["m"], tol, cfg["maxiter"])
+                    wall = time.perf_counter() - t0
+                    if best is None or info["seconds"] < best[0]["seconds"]:
+                        best = (info, wall)
+                info, wall = best
                 rows.append({"loop": name, "prec": prec, "tol": tol, "iters": info["iters"], "converged": info["converged"],
                              "ms_per_solve_device": round(1e3 * info["seconds"], 4), "ms_per_solve_wall": round(1e3 * wall, 4),
                              "us_per_iter": round(1e6 * info["seconds"] / max(info["iters"], 1), 3)})
-                ctx.close()
+            ctx.close()
     return {"lattice": list(dims), "rows": rows}
 
 

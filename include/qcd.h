@@ -219,6 +219,18 @@ long long qcd_launch_count(const qcd_ctx *ctx);
  */
 qcd_status qcd_set_dslash_variant(qcd_ctx *ctx, int variant);
 /*
+ * Solver loop of qcd_cg_solve / qcd_cg_solve_multi: all three run the same
+ * algorithm with the same per-site arithmetic; they differ in how the iterations reach the device.
+ *   0 : chosen by the library -- the persistent kernel when one right-hand side, its links and the
+ *       work vectors fit the L2 (<= 96 MB); else graph replay on small lattices when the context
+ *       stream is not the legacy default stream; else kernel-by-kernel
+ *   1 : kernel-by-kernel enqueue, the host polling the device-resident stop flag
+ *   2 : replay of a captured CUDA graph of 16 iterations (needs a non-default stream)
+ *   3 : ONE cooperative kernel runs the whole solve with grid-wide barriers between the phases
+ * Else QCD_EINVAL.
+ */
+qcd_status qcd_set_cg_loop(qcd_ctx *ctx, int mode);
+/*
  * Traversal order of the Dslash threads: the sites are walked in
  * chunks of `width` rows of x2 ((x0,x1) fastest, x2 inside the chunk, then x3, then the chunk),
  * which keeps the time-neighbour spinors of several vectors inside the L2.  A pure permutation of

@@ -33,7 +33,7 @@ SYMBOLS = [
     "qcd_field_download", "qcd_set_workspace", "qcd_dslash_eo", "qcd_dslash_oe", "qcd_apply_M",
     "qcd_cg_solve", "qcd_cg_begin", "qcd_cg_iterate", "qcd_cg_poll", "qcd_cg_finish",
     "qcd_cg_solve_host", "qcd_profile_enable", "qcd_profile_read", "qcd_launch_count",
-    "qcd_set_dslash_variant", "qcd_set_traversal_chunk", "qcd_re_dot",
+    "qcd_set_dslash_variant", "qcd_set_traversal_chunk", "qcd_set_cg_loop", "qcd_re_dot",
     # variants and mixed precision
     "qcd_gauge_compress", "qcd_gauge_fix_temporal", "qcd_gauge_set_temporal_unit", "qcd_spinor_rotate",
     "qcd_workspace_bytes_multi", "qcd_dslash_eo_multi", "qcd_dslash_oe_multi", "qcd_cg_solve_multi",
@@ -97,6 +97,7 @@ def load_library() -> ctypes.CDLL:
         "qcd_launch_count": (ctypes.c_longlong, [vp]),
         "qcd_set_dslash_variant": (ci, [vp, ci]),
         "qcd_set_traversal_chunk": (ci, [vp, ci]),
+        "qcd_set_cg_loop": (ci, [vp, ci]),
         "qcd_re_dot": (ci, [vp, vp, vp, P(cd)]),
         "qcd_gauge_compress": (ci, [vp, vp, vp]),
         "qcd_gauge_fix_temporal": (ci, [vp, vp, vp, vp]),
@@ -293,6 +294,9 @@ class Context:
 
     def qcd_set_traversal_chunk(self, width: int):
         self._check(self.lib.qcd_set_traversal_chunk(self.handle, int(width)), "qcd_set_traversal_chunk")
+
+    def qcd_set_cg_loop(self, mode: int):
+        self._check(self.lib.qcd_set_cg_loop(self.handle, int(mode)), "qcd_set_cg_loop")
 
     def qcd_re_dot(self, a: Field, b: Field) -> float:
         r = ctypes.c_double()

@@ -15,6 +15,7 @@
 #include <string>
 
 #include "cg_kernels.cuh"
+#include "cg_persistent.cuh"
 #include "dslash_launch.h"
 #include "gauge_kernels.cuh"
 #include "lattice.cuh"
@@ -66,6 +67,7 @@ struct qcd_ctx {
     CgState cg;
     int variant;
     int chunk;                // Dslash traversal chunk width in x2: 0 = automatic, else a divisor of N2
+    int loop;                 // solver loop: 0 automatic, 1 kernel-by-kernel, 2 graph replay, 3 persistent kernel
     long long launches;
     // profiling
     bool prof_on;
@@ -166,7 +168,7 @@ extern "C" qcd_status qcd_init(qcd_ctx **out, const int dims[4], int precision, 
     c->L.s1 = c->L.h; c->L.s2 = c->L.h * dims[1]; c->L.s3 = c->L.h * dims[1] * dims[2];
     c->prec = precision; c->rsize = precision == 64 ? 8 : 4;
     c->stream = (cudaStream_t)cuda_stream;
-    c->variant = 0; c->launches = 0; c->chunk = 0;
+    c->variant = 0; c->launches = 0; c->chunk = 0; c->loop = 0;
     c->L.W = dims[2];
     c->prof_on = false; c->prof_created = false; c->prof_n = c->prof_dropped = 0;
     c->ws = nullptr; c->ws_bytes = 0;
@@ -309,6 +311,14 @@ extern "C" qcd_status qcd_set_traversal_chunk(qcd_ctx *ctx, int width)
     if (!ctx) return QCD_EINVAL;
     if (width < 0 || (width > 0 && ctx->L.N2 % width)) return fail(ctx, QCD_EINVAL, "qcd_set_traversal_chunk: width must be 0 (automatic) or a divisor of N2");
     ctx->chunk = width;
+    return QCD_OK;
+}
+
+extern "C" qcd_status qcd_set_cg_loop(qcd_ctx *ctx, int mode)
+{
+    if (!ctx) return QCD_EINVAL;
+    if (mode < 0 || mode > 3) return fail(ctx, QCD_EINVAL, "qcd_set_cg_loop: mode must be 0 .. 3");
+    ctx->loop = mode;
     return QCD_OK;
 }
 
@@ -700,6 +710,52 @@ extern "C" qcd_status qcd_cg_finish(qcd_ctx *ctx, qcd_cg_info *info)
     return qcd_cg_finish_multi(ctx, info);
 }
 
+// Lattices that fit the L2: the whole solve in ONE cooperative kernel (cg_persistent.cuh).
+enum { PERSIST_MAX_BYTES = 96 << 20 };
+
+template <typename T, int NROW, int TG>
+static qcd_status cg_persistent_launch(qcd_ctx *c, bool probe_only, bool *ok)
+{
+    typedef typename Cplx<T>::type C;
+    auto kernel = cg_persistent_kernel<T, NROW, TG>;
+    int per_sm = 0, dev = 0, sms = 0, coop = 0;
+    CU(c, cudaGetDevice(&dev));
+    CU(c, cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev));
+    CU(c, cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    CU(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, PERSIST_BLOCK, 0));
+    *ok = coop && per_sm > 0;
+    if (probe_only || !*ok) return QCD_OK;
+    int grid = (c->L.Vh + PERSIST_BLOCK - 1) / PERSIST_BLOCK;
+    if (grid > per_sm * sms) grid = per_sm * sms;
+    PersistArgs<T> a;
+    a.L = c->L; a.U = (const C *)c->cg.U->ptr;
+    a.x = (C *)c->cg.x[0]; a.r = (C *)ws_r(c); a.p = (C *)ws_p(c); a.Ap = (C *)ws_Ap(c); a.t = (C *)ws_t(c);
+    a.m2 = (T)(c->cg.m * c->cg.m); a.partials = c->d_partials; a.scal = c->d_scal;
+    void *params[] = { &a };
+    LaunchScope ls(c, QCD_K_MISC);
+    CU(c, cudaLaunchCooperativeKernel((const void *)kernel, dim3(grid), dim3(PERSIST_BLOCK), params, 0, c->stream));
+    return QCD_OK;
+}
+
+static qcd_status cg_persistent(qcd_ctx *c, bool probe_only, bool *ok)
+{
+    const int nrow = gauge_nrow(c->cg.U), tg = c->cg.U->tg;
+#define QCD_PERSIST(T)                                                                                  \
+    (nrow == 3 ? (tg ? cg_persistent_launch<T, 3, 1>(c, probe_only, ok) : cg_persistent_launch<T, 3, 0>(c, probe_only, ok)) \
+               : (tg ? cg_persistent_launch<T, 2, 1>(c, probe_only, ok) : cg_persistent_launch<T, 2, 0>(c, probe_only, ok)))
+    return c->prec == 64 ? QCD_PERSIST(double) : QCD_PERSIST(float);
+#undef QCD_PERSIST
+}
+
+// the persistent kernel serves one right-hand side whose links and work vectors fit the L2
+static bool persistent_wanted(const qcd_ctx *c)
+{
+    if (c->cg.n != 1 || c->prof_on || c->loop == 1 || c->loop == 2) return false;
+    if (c->loop == 3) return true;
+    const size_t bytes = qcd_field_bytes(c, c->cg.U->kind) + 5 * half_spinor_bytes(c);
+    return bytes <= (size_t)PERSIST_MAX_BYTES;
+}
+
 // Small lattices: an iteration is 4 kernels of a few microseconds each, so the host's launch rate,
 // not the device, bounds the solve ("global reductions which have higher latencies ... more
 // pronounced for smaller lattice sizes").  There the loop replays a CUDA graph of
@@ -711,7 +767,8 @@ enum { GRAPH_ITERS = 16, GRAPH_MAX_VH = 1 << 21 };
 
 static cudaGraphExec_t cg_capture_graph(qcd_ctx *ctx)
 {
-    if (ctx->L.Vh > GRAPH_MAX_VH || ctx->prof_on || ctx->stream == nullptr || ctx->cg.maxiter < GRAPH_ITERS) return nullptr;
+    if (ctx->loop == 1 || ctx->loop == 3) return nullptr;
+    if ((ctx->L.Vh > GRAPH_MAX_VH && ctx->loop != 2) || ctx->prof_on || ctx->stream == nullptr || ctx->cg.maxiter < GRAPH_ITERS) return nullptr;
     if (cudaStreamBeginCapture(ctx->stream, cudaStreamCaptureModeThreadLocal) != cudaSuccess) { cudaGetLastError(); return nullptr; }
     const long long l0 = ctx->launches;
     const qcd_status s = qcd_cg_iterate(ctx, GRAPH_ITERS);
@@ -734,6 +791,11 @@ static cudaGraphExec_t cg_capture_graph(qcd_ctx *ctx)
 static qcd_status cg_run(qcd_ctx *ctx)
 {
     const int maxiter = ctx->cg.maxiter, n = ctx->cg.n;
+    if (persistent_wanted(ctx)) {
+        bool ok = false;
+        const qcd_status s = cg_persistent(ctx, false, &ok);
+        if (s || ok) return s;              // launched (qcd_cg_finish synchronises and reads the scalars), or failed
+    }
     int enq = 0, head = 0, tail = 0, pending = 0, chunk = 8;
     bool first = true;
     cudaGraphExec_t graph = cg_capture_graph(ctx);

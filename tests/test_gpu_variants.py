@@ -473,3 +473,67 @@ def test_traversal_chunk_is_a_pure_permutation(q, dims, prec):
     else:       # DESIGN.md R11: an fp32 solve attains what the f32 oracle variant attains, within a factor 2
         assert true <= 2.0 * max(tol, oracle.true_residual(dims, Ur, _rounded(b, prec), xo.astype(np.complex128), m)), true
     ctx.close()
+
+
+# ------------------------------------------------------------------------------------------
+# solver loop for lattices that fit the L2: one persistent cooperative kernel (qcd_set_cg_loop 3)
+# ------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("prec", [64, 32])
+@pytest.mark.parametrize("dims,links,eps,kind_name", [
+    ((16, 16, 16, 16), "near_identity", 0.3, "QCD_GAUGE"),       # configs[1]
+    ((8, 4, 6, 10), "haar", None, "QCD_GAUGE_2ROW"),             # fewer sites than resident threads, ragged
+    ((4, 4, 4, 4), "haar", None, "QCD_GAUGE"),                   # configs[0]
+    ((24, 24, 24, 24), "near_identity", 0.3, "QCD_GAUGE_2ROW"),  # more sites than resident threads: grid-stride loops
+])
+def test_cg_persistent_kernel(q, dims, links, eps, kind_name, prec):
+    """The same algorithm, the same per-site arithmetic: iteration counts equal to the kernel-by-kernel
+    loop up to the reduction order, solutions equal to rounding, oracle checks as everywhere."""
+    m = 0.05 if dims[0] >= 16 else 0.1
+    tol = 1e-10 if prec == 64 else 1e-5
+    U = qcd_inputs.gauge_field(dims, links, seed=0, eps=eps)
+    b = qcd_inputs.gaussian_source(dims, seed=1)
+    Ur, br = _rounded(U, prec), _rounded(b, prec)
+    if kind_name == "QCD_GAUGE_2ROW":
+        Ur = ov.reconstruct12(ov.compress12(Ur))
+    ctx = q.Context(dims, prec)
+    fU = ctx.field(getattr(q, kind_name)).upload(U)
+    fb, fx = ctx.field(q.QCD_SPINOR_EVEN).upload(b), ctx.field(q.QCD_SPINOR_EVEN)
+    out = {}
+    for loop in (1, 3):
+        ctx.qcd_set_cg_loop(loop)
+        n0 = ctx.qcd_launch_count()
+        info = ctx.qcd_cg_solve(fU, fb, fx, m, tol, 20000)
+        launches = ctx.qcd_launch_count() - n0
+        out[loop] = (info, fx.download().astype(np.complex128), launches)
+    (i1, x1, l1), (i3, x3, l3) = out[1], out[3]
+    assert i1["converged"] and i3["converged"]
+    assert l3 == 2 and l1 >= 4 * i1["iters"]                       # init + ONE kernel for the whole solve
+    assert abs(i1["iters"] - i3["iters"]) <= 1, (i1, i3)
+    xo, oinfo = oracle.cg(dims, Ur.astype(ctx.cdtype), br.astype(ctx.cdtype), m, tol, 20000)
+    assert iters_close(i3["iters"], oinfo["iters"]), (i3, oinfo)
+    true = oracle.true_residual(dims, Ur, br, x3, m)
+    if prec == 64:
+        assert true <= tol, true
+        assert np.linalg.norm(x3 - x1) <= 1e-9 * np.linalg.norm(x1)
+    else:
+        assert true <= 2.0 * max(tol, oracle.true_residual(dims, Ur, br, xo.astype(np.complex128), m)), true
+    # exact stop at maxiter, zero iterations, zero source
+    info = ctx.qcd_cg_solve(fU, fb, fx, m, 1e-300, 7)
+    assert info["iters"] == 7 and info["status"] == q.QCD_ENOTCONVERGED
+    x7 = fx.download()
+    ctx.qcd_set_cg_loop(1)
+    assert ctx.qcd_cg_solve(fU, fb, fx, m, 1e-300, 7)["iters"] == 7
+    assert np.allclose(fx.download(), x7, rtol=0, atol=(1e-12 if prec == 64 else 1e-5) * np.max(np.abs(x7)))
+    ctx.qcd_set_cg_loop(3)
+    info = ctx.qcd_cg_solve(fU, fb, fx, m, tol, 0)
+    assert info["iters"] == 0 and info["status"] == q.QCD_ENOTCONVERGED and not fx.download().any()
+    fz = ctx.field(q.QCD_SPINOR_EVEN)
+    fz.buf.zero_()
+    info = ctx.qcd_cg_solve(fU, fz, fx, m, tol, 100)
+    assert info["iters"] == 0 and info["converged"] and not fx.download().any()
+    # run to run bitwise reproducible
+    ctx.qcd_cg_solve(fU, fb, fx, m, tol, 20000)
+    xa = fx.download()
+    ctx.qcd_cg_solve(fU, fb, fx, m, tol, 20000)
+    assert np.array_equal(xa, fx.download())
+    ctx.close()
