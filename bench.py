@@ -499,6 +499,39 @@ def extras(args, q, torch, ctx, out, cfg, dims, U, b, fU, fb, fx, fo, peak):
                        "true_resid_oracle_fp64": oracle.true_residual(dims, U, b, xm, m),
                        "speedup_vs_cg_fp64": round(out["cg_fp64"]["s_per_solve"] / max(mi["seconds"], 1e-9), 3)}
     del xm
+    # the same two solves on the paper's link storage: temporal gauge fixed on the device,
+    # two rows stored; the source is rotated in (b' = g b), the solution rotated back (x = g^dagger x'),
+    # and the oracle checks the residual against the ORIGINAL links and source
+    fUf, fg = ctx.field(q.QCD_GAUGE), ctx.field(q.QCD_COLOUR_MATRIX)
+    ctx.qcd_gauge_fix_temporal(fU, fUf, fg)
+    f12 = ctx.field(q.QCD_GAUGE_2ROW)
+    ctx.qcd_gauge_compress(fUf, f12)
+    fUf.free()
+    g12 = c32.field(q.QCD_GAUGE_2ROW)
+    ctx.qcd_field_convert(g12, f12)
+    fbr = ctx.field(q.QCD_SPINOR_EVEN)
+    ctx.qcd_spinor_rotate(fg, fbr, fb)
+    info = ctx.qcd_cg_solve(f12, fbr, fx, m, cfg["tol64"], cfg["maxiter"])
+    ctx.qcd_spinor_rotate(fg, fx, fx, dagger=True)
+    xc = fx.download()
+    out["cg_fp64_tworow_temporal_gauge"] = {
+        "tol": cfg["tol64"], "iters": info["iters"], "converged": info["converged"], "s_per_solve": round(info["seconds"], 4),
+        "ms_per_iter": round(1e3 * info["seconds"] / max(info["iters"], 1), 5),
+        "true_resid_oracle_fp64_original_links": oracle.true_residual(dims, U, b, xc, m),
+        "speedup_vs_cg_fp64": round(out["cg_fp64"]["s_per_solve"] / max(info["seconds"], 1e-9), 3)}
+    mi = ctx.qcd_cg_solve_mixed(c32, f12, g12, fbr, fx, gx, c32.field(q.QCD_SPINOR_EVEN), m, cfg["tol64"], inner_tol,
+                                4 * cfg["maxiter"])
+    ctx.qcd_spinor_rotate(fg, fx, fx, dagger=True)
+    xc = fx.download()
+    out["cg_mixed_tworow_temporal_gauge"] = {
+        "tol": cfg["tol64"], "inner_tol": inner_tol, "converged": mi["converged"], "outer": mi["outer"],
+        "inner_iters_fp32": mi["inner_iters"], "s_per_solve": round(mi["seconds"], 4),
+        "true_resid_device_fp64": mi["true_resid"],
+        "true_resid_oracle_fp64_original_links": oracle.true_residual(dims, U, b, xc, m),
+        "speedup_vs_cg_fp64": round(out["cg_fp64"]["s_per_solve"] / max(mi["seconds"], 1e-9), 3)}
+    del xc
+    for f in (f12, g12, fg, fbr):
+        f.free()
     out["variants_fp64"] = {"lattice": list(dims), "dslash": variants_sweep(q, torch, ctx, fU, dims, peak)}
     out["cg_multi_fp64"] = cg_multi_report(q, torch, ctx.device, dims, 64, fU, m)
     # fp32: free the fp64 device fields first
