@@ -189,6 +189,36 @@ def test_cg_config1_16x16x16x16(q, prec):
 
 
 @pytest.mark.parametrize("prec", [64, 32])
+def test_dslash_config1_100_applications(q, prec):
+    """configs[1]: "100 Dslash applications".  The ORACLE builds the chain phi_{k+1} = D phi_k / 8 in fp64
+    (alternating D_oe / D_eo on a full-lattice field; 1/8 is exact and keeps the norm in range); at every
+    step the device gets the oracle's phi_k (rounded to its precision) and its D phi_k is compared with the
+    oracle's: 100 independent parity checks on vectors that become smoother and smoother eigen-mixtures."""
+    cfg, U, b = qcd_inputs.config_inputs(1)
+    dims = cfg["dims"]
+    par = qcd_inputs.site_parity(dims)
+    ctx = q.Context(dims, prec)
+    Ur = _rounded(U, prec)
+    fU = ctx.field(q.QCD_GAUGE).upload(U)
+    fin, fout = ctx.field(q.QCD_SPINOR_FULL), ctx.field(q.QCD_SPINOR_FULL)
+    phi = b.copy()                                   # even-site source
+    worst = 0.0
+    for k in range(100):
+        out_parity = 1 - (k & 1)                     # D_oe, D_eo, D_oe, ...
+        phir = _rounded(phi, prec)
+        ref = oracle.dslash(dims, Ur, phir, out_parity)
+        fin.upload(phir)
+        fout.buf.zero_()
+        (ctx.qcd_dslash_oe if out_parity else ctx.qcd_dslash_eo)(fU, fout, fin)
+        got = fout.download()
+        assert not got[par != out_parity].any()
+        worst = max(worst, dslash_rel_err(got[par == out_parity], ref[par == out_parity]))
+        phi = oracle.dslash(dims, U, phi, out_parity) / 8.0
+    assert worst <= DSLASH_TOL[prec], worst
+    ctx.close()
+
+
+@pytest.mark.parametrize("prec", [64, 32])
 @pytest.mark.parametrize("dims,links,eps", SMALL_LATTICES[1:])
 def test_cg_small_lattices(q, dims, links, eps, prec):
     m = 0.2
