@@ -115,7 +115,8 @@ qcd_status qcd_finalize(qcd_ctx *ctx);
 
 /* Bytes of a field of `kind` in the device layout above (0 for a bad kind). */
 size_t qcd_field_bytes(const qcd_ctx *ctx, int kind);
-/* Bytes of the CG workspace: 3 even + 1 odd half-fields (r, p, Ap, t = D_oe p). */
+/* Bytes of the CG workspace: 4 even + 1 odd half-fields (r, p, Ap, t = D_oe p, and a second
+ * direction buffer used by the persistent solver loop, qcd_set_cg_loop). */
 size_t qcd_workspace_bytes(const qcd_ctx *ctx);
 
 /*

@@ -9,12 +9,16 @@
 // round trip, and alpha, beta, rr, k and the stop decision are bitwise identical in all blocks,
 // so the control flow stays uniform across the grid.
 //
-//   phase 1  t  = D_oe p                                        | grid barrier
-//   phase 2  Ap = m^2 p - D_eo t;  partial Re<p,Ap> per block     | grid barrier
+//   phase 1  p' = r + beta p  (each thread for its own even site, into the OTHER p buffer) and
+//            t  = D_oe p'  with p' formed on the fly at the eight neighbours from r and p: the
+//            direction update needs no pass and no barrier of its own        | grid barrier
+//   phase 2  Ap = m^2 p' - D_eo t;  partial Re<p',Ap> per block               | grid barrier
 //            alpha = rr / sum(partials)           (every block, same order)
-//   phase 3  x += alpha p;  r -= alpha Ap;  partial <r,r>         | grid barrier
+//   phase 3  x += alpha p';  r -= alpha Ap;  partial <r,r>                    | grid barrier
 //            beta = rr' / rr;  k += 1;  stop test (every block)
-//   phase 4  p = r + beta p                                       | grid barrier
+//
+// (p' = fma(beta, p, r) gives the same bits wherever it is evaluated; beta = 0 in the first
+// iteration, where p = r = b.)
 //
 // Fields written inside the kernel (p, t, Ap, r, x) are read with L2-coherent loads (ld.global.cg),
 // never through the read-only path; links are read-only and keep it.  The arithmetic per site is
@@ -32,7 +36,7 @@ struct PersistArgs {
     typedef typename Cplx<T>::type C;
     Lattice L;
     const C *U;
-    C *x, *r, *p, *Ap, *t;     // even, even, even, even, odd half-fields
+    C *x, *r, *p, *p2, *Ap, *t; // even half-fields (p and p2 alternate as direction vector), t odd
     T m2;
     double *partials;          // 2 x gridDim.x doubles: [0] Re<p,Ap>, [1] <r,r>
     CgScalars *scal;           // initialised by cg_init_kernel (rr, bb, tol2bb, k, maxiter, flag)
@@ -42,9 +46,11 @@ __device__ __forceinline__ double2 ld_coherent(const double2 *p) { return __ldcg
 __device__ __forceinline__ float2 ld_coherent(const float2 *p) { return __ldcg(p); }
 
 // acc = (D in)(cb) for the site cb of `parity`; `in` may have been written earlier in this kernel
-template <typename T, int NROW, int TG>
+// FUSE: the input vector is r + beta * in, formed at every neighbour on the fly
+template <typename T, int NROW, int TG, bool FUSE>
 __device__ __forceinline__ void persistent_site(typename Cplx<T>::type acc[3], const Lattice &L, int parity, int cb,
-                                                const typename Cplx<T>::type *U, const typename Cplx<T>::type *in)
+                                                const typename Cplx<T>::type *U, const typename Cplx<T>::type *in,
+                                                const typename Cplx<T>::type *r = nullptr, T beta = (T)0)
 {
     typedef typename Cplx<T>::type C;
     const size_t Vh = (size_t)L.Vh;
@@ -65,6 +71,11 @@ __device__ __forceinline__ void persistent_site(typename Cplx<T>::type acc[3], c
         for (int c = 0; c < 3; ++c) {
             pf[c] = ld_coherent(in + (size_t)c * Vh + g.nf[mu]);
             pb[c] = ld_coherent(in + (size_t)c * Vh + g.nb[mu]);
+            if (FUSE) {
+                const C rf = ld_coherent(r + (size_t)c * Vh + g.nf[mu]), rb = ld_coherent(r + (size_t)c * Vh + g.nb[mu]);
+                pf[c].x = fma(beta, pf[c].x, rf.x); pf[c].y = fma(beta, pf[c].y, rf.y);
+                pb[c].x = fma(beta, pb[c].x, rb.x); pb[c].y = fma(beta, pb[c].y, rb.y);
+            }
         }
 #pragma unroll
         for (int c = 0; c < 3; ++c) {
@@ -112,23 +123,31 @@ __global__ void __launch_bounds__(PERSIST_BLOCK, 3) cg_persistent_kernel(const P
     int k = a.scal->k, flag = a.scal->flag;
     double alpha = 0.0, beta = 0.0, pAp = 0.0;
 
+    C *p_old = a.p, *p_cur = a.p2;
     while (flag == 0) {
-        // phase 1: t = D_oe p
+        // phase 1: p_cur = r + beta p_old (own even site), t = D_oe p_cur (formed on the fly at the neighbours)
+        const T be = (T)beta;
         for (int cb = gtid; cb < Vh; cb += gthreads) {
             C acc[3];
-            persistent_site<T, NROW, TG>(acc, a.L, 1, cb, a.U, a.p);
+            persistent_site<T, NROW, TG, true>(acc, a.L, 1, cb, a.U, p_old, a.r, be);
 #pragma unroll
-            for (int c = 0; c < 3; ++c) a.t[(size_t)c * sVh + cb] = acc[c];
+            for (int c = 0; c < 3; ++c) {
+                a.t[(size_t)c * sVh + cb] = acc[c];
+                C vp = ld_coherent(p_old + (size_t)c * sVh + cb);
+                const C vr = ld_coherent(a.r + (size_t)c * sVh + cb);
+                vp.x = fma(be, vp.x, vr.x); vp.y = fma(be, vp.y, vr.y);
+                p_cur[(size_t)c * sVh + cb] = vp;
+            }
         }
         grid.sync();
         // phase 2: Ap = m^2 p - D_eo t, partial Re<p,Ap>
         double dot = 0.0;
         for (int cb = gtid; cb < Vh; cb += gthreads) {
             C acc[3];
-            persistent_site<T, NROW, TG>(acc, a.L, 0, cb, a.U, a.t);
+            persistent_site<T, NROW, TG, false>(acc, a.L, 0, cb, a.U, a.t);
 #pragma unroll
             for (int c = 0; c < 3; ++c) {
-                const C vv = ld_coherent(a.p + (size_t)c * sVh + cb);
+                const C vv = ld_coherent(p_cur + (size_t)c * sVh + cb);
                 C o;
                 o.x = fma(a.m2, vv.x, -acc[c].x);
                 o.y = fma(a.m2, vv.y, -acc[c].y);
@@ -149,7 +168,7 @@ __global__ void __launch_bounds__(PERSIST_BLOCK, 3) cg_persistent_kernel(const P
         double nrm = 0.0;
         for (int i = gtid; i < 3 * Vh; i += gthreads) {
             C vx = ld_coherent(a.x + i), vr = ld_coherent(a.r + i);
-            const C vp = ld_coherent(a.p + i), va = ld_coherent(a.Ap + i);
+            const C vp = ld_coherent(p_cur + i), va = ld_coherent(a.Ap + i);
             vx.x = fma(al, vp.x, vx.x); vx.y = fma(al, vp.y, vx.y);
             vr.x = fma(-al, va.x, vr.x); vr.y = fma(-al, va.y, vr.y);
             a.x[i] = vx; a.r[i] = vr;
@@ -169,15 +188,7 @@ __global__ void __launch_bounds__(PERSIST_BLOCK, 3) cg_persistent_kernel(const P
         else if (rr_new <= tol2bb) flag = 1;
         else if (k >= maxiter) flag = 2;
         if (flag != 0) break;
-        // phase 4: p = r + beta p
-        const T be = (T)beta;
-        for (int i = gtid; i < 3 * Vh; i += gthreads) {
-            C vp = ld_coherent(a.p + i);
-            const C vr = ld_coherent(a.r + i);
-            vp.x = fma(be, vp.x, vr.x); vp.y = fma(be, vp.y, vr.y);
-            a.p[i] = vp;
-        }
-        grid.sync();
+        { C *tmp = p_old; p_old = p_cur; p_cur = tmp; }            // the direction just used becomes "p" of the next update
     }
     if (gtid == 0) {
         CgScalars *s = a.scal;

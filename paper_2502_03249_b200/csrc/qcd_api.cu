@@ -125,11 +125,13 @@ extern "C" size_t qcd_field_bytes(const qcd_ctx *ctx, int kind)
     }
 }
 
-extern "C" size_t qcd_workspace_bytes(const qcd_ctx *ctx) { return ctx ? 4 * half_spinor_bytes(ctx) : 0; }
+// r, p, Ap (even), t (odd), and a second direction buffer for the persistent kernel
+extern "C" size_t qcd_workspace_bytes(const qcd_ctx *ctx) { return ctx ? 5 * half_spinor_bytes(ctx) : 0; }
 
 extern "C" size_t qcd_workspace_bytes_multi(const qcd_ctx *ctx, int n)
 {
-    return (ctx && n >= 1 && n <= MAXRHS) ? (size_t)n * 4 * half_spinor_bytes(ctx) : 0;
+    if (!ctx || n < 1 || n > MAXRHS) return 0;
+    return n == 1 ? qcd_workspace_bytes(ctx) : (size_t)n * 4 * half_spinor_bytes(ctx);
 }
 
 static int blas_n16(const qcd_ctx *c) { return (int)(half_spinor_bytes(c) / 16); }
@@ -730,6 +732,7 @@ static qcd_status cg_persistent_launch(qcd_ctx *c, bool probe_only, bool *ok)
     PersistArgs<T> a;
     a.L = c->L; a.U = (const C *)c->cg.U->ptr;
     a.x = (C *)c->cg.x[0]; a.r = (C *)ws_r(c); a.p = (C *)ws_p(c); a.Ap = (C *)ws_Ap(c); a.t = (C *)ws_t(c);
+    a.p2 = (C *)ws_at(c, 4, 1, 0);
     a.m2 = (T)(c->cg.m * c->cg.m); a.partials = c->d_partials; a.scal = c->d_scal;
     void *params[] = { &a };
     LaunchScope ls(c, QCD_K_MISC);
@@ -752,7 +755,7 @@ static bool persistent_wanted(const qcd_ctx *c)
 {
     if (c->cg.n != 1 || c->prof_on || c->loop == 1 || c->loop == 2) return false;
     if (c->loop == 3) return true;
-    const size_t bytes = qcd_field_bytes(c, c->cg.U->kind) + 5 * half_spinor_bytes(c);
+    const size_t bytes = qcd_field_bytes(c, c->cg.U->kind) + 6 * half_spinor_bytes(c);
     return bytes <= (size_t)PERSIST_MAX_BYTES;
 }
 
