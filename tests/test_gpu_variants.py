@@ -284,6 +284,7 @@ def test_cg_multi_is_n_independent_solves(q, prec, n):
     infos = ctx.qcd_cg_solve_multi(fU, fb, fx, m, tol, 5000)
     _, oinfos = ov.cg_multi(dims, Ur.astype(ctx.cdtype), [_rounded(b, prec).astype(ctx.cdtype) for b in bs], m, tol, 5000)
     single = q.Context(dims, prec)
+    single.qcd_set_cg_loop(1)            # kernel-by-kernel: the loop the lock-step solve uses
     sU = single.field(q.QCD_GAUGE).upload(U)
     for i in range(n):
         x = fx[i].download().astype(np.complex128)
@@ -408,6 +409,7 @@ def test_cg_graph_replay_matches_plain_loop(q, prec):
         stream = torch.cuda.Stream() if use_stream else None
         with (torch.cuda.stream(stream) if use_stream else contextlib.nullcontext()):
             ctx = q.Context(dims, prec, stream=stream)
+            ctx.qcd_set_cg_loop(2 if use_stream else 1)      # graph replay / kernel-by-kernel (not the persistent kernel)
             fU = ctx.field(q.QCD_GAUGE).upload(U)
             fb = ctx.field(q.QCD_SPINOR_EVEN).upload(b)
             fx = ctx.field(q.QCD_SPINOR_EVEN)
