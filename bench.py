@@ -320,6 +320,35 @@ def small_lattice_report(q, torch, device):
     return {"lattice": list(dims), "rows": rows}
 
 
+def update_routine_report(q, torch, device, peak, dims=(48, 48, 48, 48), iters=50):
+    """The paper's Table 1 workload: bandwidth of the "CG update routine" on a 48^4 lattice,
+    fp64 -- here the fused x += alpha p, r -= alpha Ap, |r|^2 kernel (288 B per even site) and the p update
+    (144 B), timed by CUDA events around each launch inside running CG iterations."""
+    cfg, U, b = make_inputs(dims, 4)
+    Vh = int(np.prod(dims)) // 2
+    ctx = q.Context(dims, 64, device=device)
+    fU = ctx.field(q.QCD_GAUGE).upload(U)
+    fb = ctx.field(q.QCD_SPINOR_EVEN).upload(b)
+    fx = ctx.field(q.QCD_SPINOR_EVEN)
+    ctx.qcd_cg_begin(fU, fb, fx, cfg["m"], 1e-300, 1 << 30)
+    ctx.qcd_cg_iterate(5)
+    ctx.qcd_profile_enable(True)
+    ctx.qcd_cg_iterate(iters)
+    n_xr, ms_xr = ctx.qcd_profile_read(q.QCD_K_UPDATE_XR)
+    n_p, ms_p = ctx.qcd_profile_read(q.QCD_K_UPDATE_P)
+    ctx.qcd_profile_enable(False)
+    ctx.qcd_cg_finish()
+    ctx.close()
+    xr = 36 * 8 * Vh / (ms_xr / n_xr) / 1e6
+    pu = 18 * 8 * Vh / (ms_p / n_p) / 1e6
+    return {"lattice": list(dims), "update_xr_norm_ms": round(ms_xr / n_xr, 5), "update_xr_norm_gbs": round(xr, 1),
+            "update_xr_frac_of_measured_copy_peak": round(xr / peak, 4), "update_p_ms": round(ms_p / n_p, 5),
+            "update_p_gbs": round(pu, 1),
+            "paper_table1_gbs": {"OpenCL on A100": 1351, "CUDA on A100": 1317, "OpenCL on MI250x": 1134,
+                                 "peaks": {"A100": 1555, "MI250x GCD": 1638},
+                                 "source": "PAPER.md:56-62 (other hardware; context only)"}}
+
+
 def dslash_report(ms, Vh, rsize, peak):
     comp = REALS_DSLASH_COMPULSORY * rsize * Vh / ms / 1e6
     return {"ms": round(ms, 5), "gflops": round(FLOP_PER_SITE * Vh / ms / 1e6, 1),
@@ -567,6 +596,7 @@ def extras(args, q, torch, ctx, out, cfg, dims, U, b, fU, fb, fx, fo, peak):
             f.free(); c.close()
         out["variants_table2_32x32x32x32"] = t2
         out["cg_small_lattice"] = small_lattice_report(q, torch, ctx.device)
+        out["cg_update_routine_48x48x48x48"] = update_routine_report(q, torch, ctx.device, peak)
     out["paper_context"] = {"A100_OpenCL_dslash_fp64_TFLOPs_32^4_12real_links_gaugefixed": 1.245,
                             "A100_OpenCL_cg_update_GBs_48^4_fp64": 1351, "source": "PAPER.md:59,87 (other hardware; context only)"}
 

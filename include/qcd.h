@@ -215,8 +215,14 @@ qcd_status qcd_profile_read(qcd_ctx *ctx, int which, int *launches, double *tota
 long long qcd_launch_count(const qcd_ctx *ctx);
 
 /*
- * Tuning knob for the Dslash kernels (bench sweeps):
- *   variant 0 = default.  Unknown variants -> QCD_EINVAL.
+ * Tuning knob for the Dslash kernels (bench sweeps and A/B tests, Sec. 10):
+ *   0 : the library's choice (128-thread blocks, 4 resident per SM for one vector; for several vectors
+ *       the register kernel or the cp.async-staged kernel, whichever measured faster for that
+ *       (precision, number of vectors, link storage))
+ *   1, 2, 3 : one-vector kernel with 64 x 8, 256 x 2, 128 x 3 threads x resident blocks
+ *   4 : force the staged kernel (links prefetched through shared memory by cp.async)
+ *   5 : force the register kernel
+ * Every variant computes the same result (bitwise).  Unknown variants -> QCD_EINVAL.
  */
 qcd_status qcd_set_dslash_variant(qcd_ctx *ctx, int variant);
 /*
