@@ -84,7 +84,7 @@ __global__ void __launch_bounds__(BLAS_BLOCK) cg_init_kernel(
     }
     __shared__ double smem[BLAS_BLOCK / 32];
     __shared__ int last;
-    if (publish_partial<BLAS_BLOCK>(s, partials, &scal->ticket, smem, &last)) {
+    if (publish_partial<BLAS_BLOCK>(s, partials, scal, smem, &last)) {
         const double bb = final_sum<BLAS_BLOCK>(partials, (int)gridDim.x, smem);
         if (threadIdx.x == 0) {
             scal->bb = bb; scal->rr = bb; scal->tol2bb = tol * tol * bb;
@@ -103,7 +103,7 @@ template <typename T>
 __global__ void __launch_bounds__(BLAS_BLOCK) cg_update_xr_kernel(
     int n16, const __grid_constant__ RhsPtrs<typename Vec16<T>::type> ptrs, typename Vec16<T>::type *__restrict__ r,
     const typename Vec16<T>::type *__restrict__ p, const typename Vec16<T>::type *__restrict__ Ap,
-    double *partials, CgScalars *scal)
+    double *partials, CgScalars *scal, int chunks)
 {
     typedef typename Vec16<T>::type V;
     const int rhs = blockIdx.y;
@@ -114,7 +114,11 @@ __global__ void __launch_bounds__(BLAS_BLOCK) cg_update_xr_kernel(
     partials += (size_t)rhs * gridDim.x;
     const T alpha = (T)scal->alpha;
     double s = 0.0;
-    const int base = blockIdx.x * (BLAS_BLOCK * BLAS_ITEMS) + threadIdx.x;
+    // a block walks `chunks` segments and reduces once (the reduction tail, ~2 us, is then paid
+    // by a few thousand blocks instead of every 1024 vectors)
+#pragma unroll 1
+    for (int ch = 0; ch < chunks; ++ch) {
+    const int base = (blockIdx.x * chunks + ch) * (BLAS_BLOCK * BLAS_ITEMS) + threadIdx.x;
     V vx[BLAS_ITEMS], vr[BLAS_ITEMS], vp[BLAS_ITEMS], va[BLAS_ITEMS];
 #pragma unroll
     for (int j = 0; j < BLAS_ITEMS; ++j) {
@@ -131,9 +135,10 @@ __global__ void __launch_bounds__(BLAS_BLOCK) cg_update_xr_kernel(
             s += vdot(vr[j], vr[j]);
         }
     }
+    }
     __shared__ double smem[BLAS_BLOCK / 32];
     __shared__ int last;
-    if (publish_partial<BLAS_BLOCK>(s, partials, &scal->ticket, smem, &last)) {
+    if (publish_partial<BLAS_BLOCK>(s, partials, scal, smem, &last)) {
         const double rr_new = final_sum<BLAS_BLOCK>(partials, (int)gridDim.x, smem);
         if (threadIdx.x == 0) {
             scal->beta = rr_new / scal->rr;
@@ -186,7 +191,7 @@ __global__ void __launch_bounds__(BLAS_BLOCK) re_dot_kernel(
     }
     __shared__ double smem[BLAS_BLOCK / 32];
     __shared__ int last;
-    if (publish_partial<BLAS_BLOCK>(s, partials, &scal->ticket, smem, &last)) {
+    if (publish_partial<BLAS_BLOCK>(s, partials, scal, smem, &last)) {
         const double d = final_sum<BLAS_BLOCK>(partials, (int)gridDim.x, smem);
         if (threadIdx.x == 0) scal->dot = d;
     }

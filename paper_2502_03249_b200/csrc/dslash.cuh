@@ -41,6 +41,7 @@ struct DslashArgs {
     double *partials;      // MODE 2: [NRHS][gridDim.x]
     CgScalars *scal;       // MODE 2: NRHS entries (and flag source when check_flag)
     int check_flag;        // return immediately when every scal[r].flag != 0 (CG no-op iterations)
+    int chunks;            // chunks of BLOCK sites one block walks (1 unless MODE 2, see dslash_kernel)
 };
 
 // acc += U * p
@@ -165,7 +166,7 @@ __device__ __forceinline__ void dslash_reduce(const DslashArgs<T, NRHS> &a, doub
     if (MODE == 2) {
         __shared__ double smem[NRHS * (BLOCK / 32)];
         __shared__ int last;
-        if (publish_partials<BLOCK, NRHS>(dot, a.partials, (size_t)gridDim.x, &a.scal[0].ticket, smem, &last)) {
+        if (publish_partials<BLOCK, NRHS>(dot, a.partials, (size_t)gridDim.x, a.scal, smem, &last)) {
             for (int r = 0; r < NRHS; ++r) {
                 const double pAp = final_sum<BLOCK>(a.partials + (size_t)r * gridDim.x, (int)gridDim.x, smem);
                 if (threadIdx.x == 0) {
@@ -193,14 +194,20 @@ __global__ void __launch_bounds__(BLOCK, MINB) dslash_kernel(const DslashArgs<T,
         if (all_done) return;
     }
 
-    const int tid = blockIdx.x * BLOCK + threadIdx.x;
-    const bool active = tid < a.L.Vh;
-    const int cb = active ? traversal_site(a.L, tid) : tid;
     const size_t Vh = (size_t)a.L.Vh;
     double dot[NRHS];
 #pragma unroll
     for (int r = 0; r < NRHS; ++r) dot[r] = 0.0;
 
+    // MODE 2 ends every block with a reduction (two block barriers, a fence, a ticket): ~2 us during
+    // which the block's registers sit idle -- 25 % of a block that handles one site per thread in
+    // fp32.  A block therefore walks a.chunks chunks of BLOCK sites and reduces once; the host sizes
+    // the grid to a few thousand blocks (dslash_inst.cuh).
+#pragma unroll 1
+    for (int chunk = 0; chunk < (MODE == 2 ? a.chunks : 1); ++chunk) {
+    const int tid = (blockIdx.x * (MODE == 2 ? a.chunks : 1) + chunk) * BLOCK + threadIdx.x;
+    const bool active = tid < a.L.Vh;
+    const int cb = active ? traversal_site(a.L, tid) : tid;
     if (active) {
         const SiteGeom g = site_geometry(a.L, a.parity, cb);
         const uint64_t pol_stream = l2_policy_evict_first();
@@ -212,6 +219,14 @@ __global__ void __launch_bounds__(BLOCK, MINB) dslash_kernel(const DslashArgs<T,
 #pragma unroll
         for (int r = 0; r < NRHS; ++r)
             acc[r][0].x = acc[r][0].y = acc[r][1].x = acc[r][1].y = acc[r][2].x = acc[r][2].y = (T)0;
+        if (MODE >= 1) {
+            // the epilogue reads v(x) after the last hop, when nothing is left to hide a DRAM round
+            // trip behind: ask the L2 for it now (no register is held)
+#pragma unroll
+            for (int r = 0; r < NRHS; ++r)
+#pragma unroll
+                for (int c = 0; c < 3; ++c) prefetch_l2(a.v[r] + (size_t)c * Vh + cb);
+        }
 
 #pragma unroll
         for (int mu = 0; mu < 4; ++mu) {
@@ -272,6 +287,7 @@ __global__ void __launch_bounds__(BLOCK, MINB) dslash_kernel(const DslashArgs<T,
 
         dslash_epilogue<T, MODE, NRHS>(a, cb, acc, dot);
     }
+    }
     dslash_reduce<T, MODE, NRHS, BLOCK>(a, dot);
 }
 
@@ -299,14 +315,16 @@ __global__ void __launch_bounds__(BLOCK, MINB) dslash_staged_kernel(const Dslash
         if (all_done) return;
     }
 
-    const int tid = blockIdx.x * BLOCK + threadIdx.x;
-    const bool active = tid < a.L.Vh;
-    const int cb = active ? traversal_site(a.L, tid) : tid;
     const size_t Vh = (size_t)a.L.Vh;
     double dot[NRHS];
 #pragma unroll
     for (int r = 0; r < NRHS; ++r) dot[r] = 0.0;
 
+#pragma unroll 1
+    for (int chunk = 0; chunk < (MODE == 2 ? a.chunks : 1); ++chunk) {
+    const int tid = (blockIdx.x * (MODE == 2 ? a.chunks : 1) + chunk) * BLOCK + threadIdx.x;
+    const bool active = tid < a.L.Vh;
+    const int cb = active ? traversal_site(a.L, tid) : tid;
     if (active) {
         const SiteGeom g = site_geometry(a.L, a.parity, cb);
         const uint64_t pol_stream = l2_policy_evict_first();
@@ -379,6 +397,7 @@ __global__ void __launch_bounds__(BLOCK, MINB) dslash_staged_kernel(const Dslash
             if (h + DEPTH < 8) issue(h + DEPTH);
         }
         dslash_epilogue<T, MODE, NRHS>(a, cb, acc, dot);
+    }
     }
     dslash_reduce<T, MODE, NRHS, BLOCK>(a, dot);
 }

@@ -26,6 +26,19 @@ template <> struct DslashCfg<float, 6> { enum { BLOCK = 128, MINB = 3 }; };
 template <> struct DslashCfg<float, 7> { enum { BLOCK = 128, MINB = 2 }; };
 template <> struct DslashCfg<float, 8> { enum { BLOCK = 128, MINB = 2 }; };
 
+// Kernels that end with a block reduction (MODE 2) walk several chunks of BLOCK sites per block so
+// that the ~2 us reduction tail is paid once per several hundred sites, not by every 128: the grid
+// is sized to about REDUCE_GRID blocks (32 waves of 148 SMs x 4 resident blocks; 4 chunks per block
+// at 64^4).  Measured at 64^4: fewer, longer blocks (14 chunks) lose more in the last wave than they
+// save (fp64 epilogue kernel 1.58 -> 1.68 ms), and a grid-stride order of the chunks is slower still.
+enum { REDUCE_GRID = 148 * 4 * 32 };
+static inline int reduce_chunks(int Vh, int block)
+{
+    const int blocks = (Vh + block - 1) / block;
+    const int c = (blocks + REDUCE_GRID - 1) / REDUCE_GRID;
+    return c < 1 ? 1 : c;
+}
+
 template <typename T, int MODE, int NROW, int TG, int NRHS, int BLOCK, int MINB>
 static cudaError_t launch_cfg(const DslashLaunch &d)
 {
@@ -34,7 +47,9 @@ static cudaError_t launch_cfg(const DslashLaunch &d)
     a.L = d.L; a.parity = d.parity; a.U = (const C *)d.U;
     for (int r = 0; r < NRHS; ++r) { a.in[r] = (const C *)d.in[r]; a.out[r] = (C *)d.out[r]; a.v[r] = (const C *)d.v[r]; }
     a.m2 = (T)d.m2; a.partials = d.partials; a.scal = d.scal; a.check_flag = d.check_flag;
-    const int grid = (d.L.Vh + BLOCK - 1) / BLOCK;
+    a.chunks = MODE == 2 ? reduce_chunks(d.L.Vh, BLOCK) : 1;
+    const int per_block = BLOCK * a.chunks;
+    const int grid = (d.L.Vh + per_block - 1) / per_block;
     dslash_kernel<T, MODE, NROW, TG, NRHS, BLOCK, MINB><<<grid, BLOCK, 0, d.stream>>>(a);
     return cudaGetLastError();
 }
@@ -60,7 +75,9 @@ static cudaError_t launch_staged(const DslashLaunch &d)
     a.L = d.L; a.parity = d.parity; a.U = (const C *)d.U;
     for (int r = 0; r < NRHS; ++r) { a.in[r] = (const C *)d.in[r]; a.out[r] = (C *)d.out[r]; a.v[r] = (const C *)d.v[r]; }
     a.m2 = (T)d.m2; a.partials = d.partials; a.scal = d.scal; a.check_flag = d.check_flag;
-    const int grid = (d.L.Vh + BLOCK - 1) / BLOCK;
+    a.chunks = MODE == 2 ? reduce_chunks(d.L.Vh, BLOCK) : 1;
+    const int per_block = BLOCK * a.chunks;
+    const int grid = (d.L.Vh + per_block - 1) / per_block;
     kernel<<<grid, BLOCK, smem, d.stream>>>(a);
     return cudaGetLastError();
 }

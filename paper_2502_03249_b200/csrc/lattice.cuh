@@ -83,6 +83,8 @@ __device__ __forceinline__ float4 ld_keep(const float4 *p, uint64_t pol)
     return r;
 }
 
+__device__ __forceinline__ void prefetch_l2(const void *p) { asm volatile("prefetch.global.L2 [%0];" :: "l"(p)); }
+
 // Asynchronous global -> shared copies (LDGSTS): the data never passes through registers, so a
 // thread can keep many link loads in flight without holding registers for them.  16-byte copies
 // bypass L1 (.cg); 8-byte copies exist only as .ca.  L2 policy operand as for ld_stream.

@@ -32,7 +32,7 @@ __global__ void __launch_bounds__(BLAS_BLOCK) mixed_residual_kernel(
     }
     __shared__ double smem[BLAS_BLOCK / 32];
     __shared__ int last;
-    if (publish_partial<BLAS_BLOCK>(s, partials, &scal->ticket, smem, &last)) {
+    if (publish_partial<BLAS_BLOCK>(s, partials, scal, smem, &last)) {
         const double d = final_sum<BLAS_BLOCK>(partials, (int)gridDim.x, smem);
         if (threadIdx.x == 0) scal->dot = d;
     }

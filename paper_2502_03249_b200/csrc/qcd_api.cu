@@ -58,6 +58,7 @@ struct qcd_ctx {
     CgScalars *d_scal;        // CG recurrence state, MAXRHS entries
     CgScalars *d_aux;         // scratch state for qcd_apply_M / qcd_re_dot / the mixed solver
     double *d_partials;       // stage-1 partial sums
+    unsigned *d_tickets;      // first-level tickets of the two-level last-block election (reduce.cuh)
     int partials_cap;
     CgScalars *h_scal;        // pinned, POLL_SLOTS x MAXRHS entries
     cudaEvent_t poll_ev[POLL_SLOTS];
@@ -134,6 +135,8 @@ extern "C" size_t qcd_workspace_bytes_multi(const qcd_ctx *ctx, int n)
     return n == 1 ? qcd_workspace_bytes(ctx) : (size_t)n * 4 * half_spinor_bytes(ctx);
 }
 
+// target grid of the reducing vector kernel (8 waves of 148 SMs x 8 resident blocks of 256 threads)
+enum { BLAS_REDUCE_GRID = 148 * 8 * 8 };
 static int blas_n16(const qcd_ctx *c) { return (int)(half_spinor_bytes(c) / 16); }
 static int blas_grid(const qcd_ctx *c) { const int per = BLAS_BLOCK * BLAS_ITEMS; return (blas_n16(c) + per - 1) / per; }
 static int dslash_grid_max(const qcd_ctx *c) { return (c->L.Vh + 63) / 64; }   // smallest Dslash block is 64
@@ -175,7 +178,7 @@ extern "C" qcd_status qcd_init(qcd_ctx **out, const int dims[4], int precision, 
     c->prof_on = false; c->prof_created = false; c->prof_n = c->prof_dropped = 0;
     c->ws = nullptr; c->ws_bytes = 0;
     memset(&c->cg, 0, sizeof c->cg);
-    c->d_scal = c->d_aux = nullptr; c->d_partials = nullptr; c->h_scal = nullptr; c->d_stage = nullptr;
+    c->d_scal = c->d_aux = nullptr; c->d_partials = nullptr; c->d_tickets = nullptr; c->h_scal = nullptr; c->d_stage = nullptr;
     for (int i = 0; i < POLL_SLOTS; ++i) c->poll_ev[i] = nullptr;
 
     c->partials_cap = MAXRHS * (dslash_grid_max(c) > blas_grid(c) ? dslash_grid_max(c) : blas_grid(c));
@@ -183,6 +186,13 @@ extern "C" qcd_status qcd_init(qcd_ctx **out, const int dims[4], int precision, 
     if (err == cudaSuccess) err = cudaMalloc(&c->d_scal, (MAXRHS + 1) * sizeof(CgScalars));
     if (err == cudaSuccess) err = cudaMemset(c->d_scal, 0, (MAXRHS + 1) * sizeof(CgScalars));
     if (err == cudaSuccess) err = cudaMalloc(&c->d_partials, (size_t)c->partials_cap * sizeof(double));
+    const size_t groups = (size_t)(c->partials_cap / MAXRHS) / TICKET_GROUP + 1;      // per CgScalars entry
+    if (err == cudaSuccess) err = cudaMalloc(&c->d_tickets, (MAXRHS + 1) * groups * sizeof(unsigned));
+    if (err == cudaSuccess) err = cudaMemset(c->d_tickets, 0, (MAXRHS + 1) * groups * sizeof(unsigned));
+    for (int i = 0; i <= MAXRHS && err == cudaSuccess; ++i) {
+        unsigned *l1 = c->d_tickets + (size_t)i * groups;
+        err = cudaMemcpy(&c->d_scal[i].l1, &l1, sizeof l1, cudaMemcpyHostToDevice);
+    }
     if (err == cudaSuccess) err = cudaMalloc(&c->d_stage, STAGE_BYTES);
     if (err == cudaSuccess) err = cudaMallocHost(&c->h_scal, POLL_SLOTS * MAXRHS * sizeof(CgScalars));
     for (int i = 0; i < POLL_SLOTS && err == cudaSuccess; ++i) err = cudaEventCreateWithFlags(&c->poll_ev[i], cudaEventDisableTiming);
@@ -208,6 +218,7 @@ extern "C" qcd_status qcd_finalize(qcd_ctx *c)
     if (c->cg.ev_end) cudaEventDestroy(c->cg.ev_end);
     if (c->d_scal) cudaFree(c->d_scal);
     if (c->d_partials) cudaFree(c->d_partials);
+    if (c->d_tickets) cudaFree(c->d_tickets);
     if (c->d_stage) cudaFree(c->d_stage);
     if (c->h_scal) cudaFreeHost(c->h_scal);
     delete c;
@@ -586,8 +597,9 @@ static qcd_status cg_iteration_t(qcd_ctx *c)
     if (s) return s;
     {
         LaunchScope ls(c, QCD_K_UPDATE_XR);
-        cg_update_xr_kernel<T><<<dim3(blas_grid(c), n), BLAS_BLOCK, 0, c->stream>>>(
-            blas_n16(c), rhs_ptrs<T>(c), (V *)ws_r(c, n), (const V *)ws_p(c, n), (const V *)ws_Ap(c, n), c->d_partials, c->d_scal);
+        const int chunks = (blas_grid(c) + BLAS_REDUCE_GRID - 1) / BLAS_REDUCE_GRID;          // >= 1
+        cg_update_xr_kernel<T><<<dim3((blas_grid(c) + chunks - 1) / chunks, n), BLAS_BLOCK, 0, c->stream>>>(
+            blas_n16(c), rhs_ptrs<T>(c), (V *)ws_r(c, n), (const V *)ws_p(c, n), (const V *)ws_Ap(c, n), c->d_partials, c->d_scal, chunks);
     }
     {
         LaunchScope ls(c, QCD_K_UPDATE_P);
