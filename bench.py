@@ -375,16 +375,31 @@ def run_ours(args):
     K, W = args.steps, args.warmup
     peak, peak_src = load_peaks()
     t_setup = time.time()
-    cfg, U, b = make_inputs(dims)
     V = int(np.prod(dims))
     Vh = V // 2
-    m, tol64 = cfg["m"], cfg["tol64"]
-
     ctx = q.Context(dims, 64, device=dev)
-    fU = ctx.field(q.QCD_GAUGE).upload(U)
-    fb = ctx.field(q.QCD_SPINOR_EVEN).upload(b)
+    fU = ctx.field(q.QCD_GAUGE)
+    fb = ctx.field(q.QCD_SPINOR_EVEN)
     fx = ctx.field(q.QCD_SPINOR_EVEN)
     fo = ctx.field(q.QCD_SPINOR_ODD)
+    if rank == 0:
+        cfg, U, b = make_inputs(dims)
+        fU.upload(U)
+        fb.upload(b)
+    else:
+        # replicas: every rank works on the SAME inputs.  Rank 0 generates them (9.7 GB of links on the
+        # host) and the device images are broadcast once during set-up -- plumbing, outside every timed
+        # region; eight ranks generating 64^4 on one host would need ~200 GB of host memory.
+        import qcd_inputs
+        cfg, U, b = dict(qcd_inputs.CONFIGS[4]), None, None
+        cfg["dims"] = tuple(dims)
+    if world > 1:
+        import torch.distributed as dist
+        dist.broadcast(fU.buf, src=0)
+        dist.broadcast(fb.buf, src=0)
+        if rank != 0:
+            b = fb.download()                  # the canonical host source (for the e2e leg) through the library
+    m, tol64 = cfg["m"], cfg["tol64"]
     t_setup = time.time() - t_setup
 
     def barrier():
