@@ -320,6 +320,58 @@ def small_lattice_report(q, torch, device):
     return {"lattice": list(dims), "rows": rows}
 
 
+FLOP_PER_CG_ITER = 2 * FLOP_PER_SITE + 72     # per even site: two half-Dslash + m^2 p - (6 fma) + two dots (2 x 12) + x, r, p updates (3 x 12)
+
+
+def size_sweep_report(q, torch, device, sizes=((8, 8, 8, 8), (12, 12, 12, 12), (16, 16, 16, 16), (24, 24, 24, 24),
+                                               (32, 32, 32, 32), (48, 48, 48, 12)), iters=200):
+    """The paper's Fig. 3 experiment: Dslash and CG throughput against the lattice size, in
+    single and double precision (the 64^4 point is the headline above).  Dslash: 20 back-to-back D_oe launches;
+    CG: qcd_cg_solve with an unreachable tolerance and maxiter = `iters`, i.e. the solver loop the library picks
+    for that size (persistent kernel while the lattice fits the L2, kernel-by-kernel beyond).  GFLOP/s with
+    570 flop per site (Dslash) and 2 x 570 + 72 flop per even site and iteration (CG)."""
+    import qcd_inputs
+    rows = []
+    for dims in sizes:
+        Vh = int(np.prod(dims)) // 2
+        U = qcd_inputs.gauge_field(dims, "haar", seed=0)
+        b = qcd_inputs.gaussian_source(dims, seed=1)
+        for prec in (64, 32):
+            stream = torch.cuda.Stream(device=device)
+            with torch.cuda.stream(stream):
+                ctx = q.Context(dims, prec, device=device, stream=stream)
+                fU = ctx.field(q.QCD_GAUGE).upload(U)
+                fb = ctx.field(q.QCD_SPINOR_EVEN).upload(b)
+                fx = ctx.field(q.QCD_SPINOR_EVEN)
+                fo = ctx.field(q.QCD_SPINOR_ODD)
+                # 20 launches captured in one CUDA graph: below 16^4 a Python-driven launch loop would
+                # time the host, not the kernel
+                ctx.qcd_dslash_oe(fU, fo, fb)
+                stream.synchronize()
+                graph = torch.cuda.CUDAGraph()
+                with torch.cuda.graph(graph, stream=stream):
+                    for _ in range(20):
+                        ctx.qcd_dslash_oe(fU, fo, fb)
+                graph.replay()
+                stream.synchronize()
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record(stream)
+                for _ in range(5):
+                    graph.replay()
+                e1.record(stream)
+                stream.synchronize()
+                ms_d = e0.elapsed_time(e1) / 100
+                del graph
+            ctx.qcd_cg_solve(fU, fb, fx, 0.01, 1e-300, 20)
+            secs = min(ctx.qcd_cg_solve(fU, fb, fx, 0.01, 1e-300, iters)["seconds"] for _ in range(2))
+            rows.append({"lattice": list(dims), "prec": prec, "dslash_us": round(1e3 * ms_d, 3),
+                         "dslash_gflops": round(FLOP_PER_SITE * Vh / ms_d / 1e6, 1),
+                         "cg_us_per_iter": round(1e6 * secs / iters, 3),
+                         "cg_gflops": round(FLOP_PER_CG_ITER * Vh * iters / secs / 1e9, 1)})
+            ctx.close()
+    return rows
+
+
 def update_routine_report(q, torch, device, peak, dims=(48, 48, 48, 48), iters=50):
     """The paper's Table 1 workload: bandwidth of the "CG update routine" on a 48^4 lattice,
     fp64 -- here the fused x += alpha p, r -= alpha Ap, |r|^2 kernel (288 B per even site) and the p update
@@ -612,6 +664,7 @@ def extras(args, q, torch, ctx, out, cfg, dims, U, b, fU, fb, fx, fo, peak):
         out["variants_table2_32x32x32x32"] = t2
         out["cg_small_lattice"] = small_lattice_report(q, torch, ctx.device)
         out["cg_update_routine_48x48x48x48"] = update_routine_report(q, torch, ctx.device, peak)
+        out["size_sweep_fig3"] = size_sweep_report(q, torch, ctx.device)
     out["paper_context"] = {"A100_OpenCL_dslash_fp64_TFLOPs_32^4_12real_links_gaugefixed": 1.245,
                             "A100_OpenCL_cg_update_GBs_48^4_fp64": 1351, "source": "PAPER.md:59,87 (other hardware; context only)"}
 
