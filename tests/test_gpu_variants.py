@@ -539,3 +539,60 @@ def test_cg_persistent_kernel(q, dims, links, eps, kind_name, prec):
     ctx.qcd_cg_solve(fU, fb, fx, m, tol, 20000)
     assert np.array_equal(xa, fx.download())
     ctx.close()
+
+
+# ------------------------------------------------------------------------------------------
+# index arithmetic on unusual shapes: seeded random extents, every kernel family
+# ------------------------------------------------------------------------------------------
+def _random_shapes(n, seed=5):
+    rng = np.random.default_rng(seed)
+    shapes = [(4, 2, 2, 2), (4, 2, 2, 12), (16, 2, 6, 2), (20, 4, 2, 4)]        # extremes first: h = 2, N = 2 everywhere
+    while len(shapes) < n:
+        shapes.append((int(rng.choice([4, 8, 12, 16, 20, 24])), int(rng.choice([2, 4, 6, 8, 10])),
+                       int(rng.choice([2, 4, 6, 8])), int(rng.choice([2, 4, 6, 10, 14]))))
+    return shapes
+
+
+@pytest.mark.parametrize("dims", _random_shapes(12))
+def test_random_shapes_every_kernel_family(q, dims):
+    """Full links / two rows / two rows + temporal gauge, 1 and 3 vectors (register, staged), both
+    precisions, D_oe and D_eo, against the oracle; then a CG solve in each solver loop."""
+    U = qcd_inputs.gauge_field(dims, "haar", seed=0)
+    Ufix, _ = ov.temporal_gauge(dims, U)
+    Ufix[qcd_inputs.site_coords(dims)[:, 3] != 0, 3] = np.eye(3)
+    phis = [qcd_inputs.gaussian_spinor(dims, seed=60 + i) for i in range(3)]
+    par = qcd_inputs.site_parity(dims)
+    for prec in (64, 32):
+        ctx = q.Context(dims, prec, nrhs=3)
+        fin = [ctx.field(q.QCD_SPINOR_FULL).upload(p) for p in phis]
+        fout = [ctx.field(q.QCD_SPINOR_FULL) for _ in phis]
+        for kind, links, tg in ((q.QCD_GAUGE, U, False), (q.QCD_GAUGE_2ROW, U, False), (q.QCD_GAUGE_2ROW, Ufix, True)):
+            fU = ctx.field(kind).upload(links)
+            ctx.qcd_gauge_set_temporal_unit(fU, tg)
+            Ur = _rounded(links, prec)
+            if kind == q.QCD_GAUGE_2ROW:
+                Ur = ov.reconstruct12(ov.compress12(Ur))
+            refs = [oracle.dslash(dims, Ur, _rounded(p, prec), -1) for p in phis]
+            for n in (1, 3):
+                for f in fout:
+                    f.buf.zero_()
+                ctx.qcd_dslash_eo_multi(fU, fout[:n], fin[:n])
+                ctx.qcd_dslash_oe_multi(fU, fout[:n], fin[:n])
+                for i in range(n):
+                    got = fout[i].download()
+                    for p in (0, 1):
+                        assert dslash_rel_err(got[par == p], refs[i][par == p]) <= DSLASH_TOL[prec], (prec, kind, tg, n, i, p)
+        # CG on the full links, every solver loop
+        b = qcd_inputs.gaussian_source(dims, seed=1)
+        m, tol = 0.2, (1e-9 if prec == 64 else 1e-5)
+        fU = ctx.field(q.QCD_GAUGE).upload(U)
+        fb, fx = ctx.field(q.QCD_SPINOR_EVEN).upload(b), ctx.field(q.QCD_SPINOR_EVEN)
+        Ur, br = _rounded(U, prec), _rounded(b, prec)
+        xo, oinfo = oracle.cg(dims, Ur.astype(ctx.cdtype), br.astype(ctx.cdtype), m, tol, 3000)
+        bound = tol if prec == 64 else 2.0 * max(tol, oracle.true_residual(dims, Ur, br, xo.astype(np.complex128), m))
+        for loop in (1, 3):
+            ctx.qcd_set_cg_loop(loop)
+            info = ctx.qcd_cg_solve(fU, fb, fx, m, tol, 3000)
+            assert info["converged"] and iters_close(info["iters"], oinfo["iters"]), (prec, loop, info, oinfo)
+            assert oracle.true_residual(dims, Ur, br, fx.download().astype(np.complex128), m) <= bound, (prec, loop)
+        ctx.close()
