@@ -63,7 +63,9 @@ def parse_args():
     ap.add_argument("--quick", action="store_true", help="skip the extra reports (full solves, fp32, cpu_baseline)")
     ap.add_argument("--variants-only", action="store_true",
                     help="run only the Dslash variant sweep (two-row / temporal gauge / NMULTI) and print it; used for ncu captures")
-    ap.add_argument("--prec", type=int, default=64, choices=(64, 32), help="precision of --variants-only")
+    ap.add_argument("--prec", type=int, default=64, choices=(64, 32),
+                    help="precision of --variants-only, and of the timed CG iterations (32: the fp32 path of the same "
+                         "workload, reported with dtype f32 and without the extra reports; the default line is fp64)")
     ap.add_argument("--nmulti", default="1,2,3,4,6,8", help="NMULTI values of --variants-only")
     ap.add_argument("--reps", type=int, default=10, help="timed launches per variant of --variants-only")
     ap.add_argument("--kernel", type=int, default=0,
@@ -429,7 +431,9 @@ def run_ours(args):
     t_setup = time.time()
     V = int(np.prod(dims))
     Vh = V // 2
-    ctx = q.Context(dims, 64, device=dev)
+    prec = args.prec
+    rsize = prec // 8
+    ctx = q.Context(dims, prec, device=dev)
     fU = ctx.field(q.QCD_GAUGE)
     fb = ctx.field(q.QCD_SPINOR_EVEN)
     fx = ctx.field(q.QCD_SPINOR_EVEN)
@@ -481,12 +485,12 @@ def run_ours(args):
     ctx.qcd_cg_finish()
     assert state == 0 and it_done == W + K, (state, it_done)
 
-    bytes_iter = REALS_ITER_NOMINAL * 8 * Vh
+    bytes_iter = REALS_ITER_NOMINAL * rsize * Vh
     ms_max, units = aggregate_over_ranks(ms_total, float(K) * bytes_iter, dev if world > 1 else None)
     value = units / ms_max / 1e6
 
     # ---------------- e2e: host buffers through the C-ABI --------------------------------------
-    hb = torch.from_numpy(b).pin_memory()
+    hb = torch.from_numpy(np.ascontiguousarray(b, dtype=ctx.cdtype)).pin_memory()
     hx = torch.empty_like(hb).pin_memory()
     torch.cuda.synchronize()
     barrier()
@@ -516,11 +520,11 @@ def run_ours(args):
     # ---------------- roofline of the dominant kernel ------------------------------------------
     n_ds, ms_ds = prof[q.QCD_K_DSLASH]
     ds_ms = ms_ds / max(n_ds, 1)
-    achieved = REALS_DSLASH_COMPULSORY * 8 * Vh / ds_ms / 1e6
-    roofline = {"bound": "hbm", "kernel": "dslash_kernel<double,MODE0> (D_oe inside the CG iteration)",
+    achieved = REALS_DSLASH_COMPULSORY * rsize * Vh / ds_ms / 1e6
+    roofline = {"bound": "hbm", "kernel": f"dslash_kernel<{'double' if prec == 64 else 'float'},MODE0> (D_oe inside the CG iteration)",
                 "achieved": round(achieved, 1), "peak": peak, "unit": "GB/s", "frac": round(achieved / peak, 4),
-                "peak_source": peak_src, "traffic": load_traffic(64) if dims == (64, 64, 64, 64) else None,
-                "algorithmic_bytes_per_launch": REALS_DSLASH_COMPULSORY * 8 * Vh,
+                "peak_source": peak_src, "traffic": load_traffic(prec) if dims == (64, 64, 64, 64) else None,
+                "algorithmic_bytes_per_launch": REALS_DSLASH_COMPULSORY * rsize * Vh,
                 "avg_launch_ms": round(ds_ms, 5), "launches_timed": n_ds,
                 "frac_of_theoretical_8184": round(achieved / THEORETICAL_HBM_GBS, 4)}
     kernel_ms = {name: round(prof[k][1] / max(prof[k][0], 1), 5) for name, k in
@@ -528,18 +532,19 @@ def run_ours(args):
                   ("update_xr_norm", q.QCD_K_UPDATE_XR), ("update_p", q.QCD_K_UPDATE_P))}
 
     out = {
-        "metric": METRIC, "value": round(value, 2), "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+        "metric": METRIC if prec == 64 else METRIC.replace("fp64", "fp32").replace("1584", "792"),
+        "value": round(value, 2), "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
         "ms_per_step": round(ms_max / K, 5), "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-        "dtype": "f64", "data": "synthetic (seeded Haar SU(3) links, Gaussian source; BASELINE.json configs[4])",
-        "config": {"workload": f"{'x'.join(map(str, dims))} staggered CG iteration, Haar links, m={m}, fp64, full 18-real links",
+        "dtype": f"f{prec}", "data": "synthetic (seeded Haar SU(3) links, Gaussian source; BASELINE.json configs[4])",
+        "config": {"workload": f"{'x'.join(map(str, dims))} staggered CG iteration, Haar links, m={m}, fp{prec}, full 18-real links",
                    "lattice": list(dims), "sites": V, "l2": "inputs (9.7 GB links) >> 126 MB L2, no flush needed",
                    "parallelism": "replicas only (no data-path collective)" if world > 1 else "single GPU",
-                   "bytes_per_even_site_per_step": REALS_ITER_NOMINAL * 8},
+                   "bytes_per_even_site_per_step": REALS_ITER_NOMINAL * rsize},
         "clocks": clocks.summary(), "e2e": e2e, "gpu_launches": int(launches),
         "roofline": roofline, "kernel_ms": kernel_ms, "setup_seconds": round(t_setup, 1),
     }
 
-    if rank == 0 and not args.quick:
+    if rank == 0 and not args.quick and prec == 64:
         extras(args, q, torch, ctx, out, cfg, dims, U, b, fU, fb, fx, fo, peak)
     if rank == 0:
         print(json.dumps(out), flush=True)
