@@ -590,7 +590,7 @@ def extras(args, q, torch, ctx, out, cfg, dims, U, b, fU, fb, fx, fo, peak):
     gx = c32.field(q.QCD_SPINOR_EVEN)
     go = c32.field(q.QCD_SPINOR_ODD)
     # mixed-precision defect-correction CG to the fp64 tolerance (R21)
-    inner_tol = 1e-2
+    inner_tol = 1e-3
     mi = ctx.qcd_cg_solve_mixed(c32, fU, gU, fb, fx, gx, c32.field(q.QCD_SPINOR_EVEN), m, cfg["tol64"], inner_tol,
                                 4 * cfg["maxiter"])
     xm = fx.download()
