@@ -224,3 +224,24 @@ def test_cg_full_size(q, config, prec):
     assert g["tol"] == tol and g["m"] == m and g["status"] == 0
     assert iters_close(info["iters"], g["iters"]), (info["iters"], g["iters"])
     assert abs(info["bnorm2"] - g["bnorm2"]) <= 1e-6 * g["bnorm2"]
+
+
+@pytest.mark.parametrize("config,prec", [(2, 64), (4, 32)])
+def test_cg_full_size_is_bitwise_reproducible(q, config, prec):
+    """The reductions are deterministic (fixed summation order, integer tickets only): two solves of the
+    same system give the same iteration count, the same recurrence residual and the same bits in x."""
+    cfg, U, b = inputs(config)
+    dims, m = cfg["dims"], cfg["m"]
+    tol = cfg["tol64"] if prec == 64 else cfg["tol32"]
+    ctx = q.Context(dims, prec)
+    fU = ctx.field(q.QCD_GAUGE).upload(U)
+    fb = ctx.field(q.QCD_SPINOR_EVEN).upload(b)
+    fx = ctx.field(q.QCD_SPINOR_EVEN)
+    i1 = ctx.qcd_cg_solve(fU, fb, fx, m, tol, cfg["maxiter"])
+    x1 = fx.download()
+    fx.buf.zero_()
+    i2 = ctx.qcd_cg_solve(fU, fb, fx, m, tol, cfg["maxiter"])
+    x2 = fx.download()
+    ctx.close()
+    assert i1["iters"] == i2["iters"] and i1["rel_resid"] == i2["rel_resid"]
+    assert np.array_equal(x1, x2)
