@@ -521,12 +521,18 @@ def run_ours(args):
     n_ds, ms_ds = prof[q.QCD_K_DSLASH]
     ds_ms = ms_ds / max(n_ds, 1)
     achieved = REALS_DSLASH_COMPULSORY * rsize * Vh / ds_ms / 1e6
+    # read-only streaming ceiling over the gauge field's own bytes (qcd_stream_read: the Dslash's link-load
+    # instruction and nothing else), measured after the timed region; the third denominator beside the
+    # copy peak and the theoretical peak
+    ctx.qcd_stream_read(fU, 3)
+    stream_gbs = fU.nbytes / ctx.qcd_stream_read(fU, 10) / 1e6
     roofline = {"bound": "hbm", "kernel": f"dslash_kernel<{'double' if prec == 64 else 'float'},MODE0> (D_oe inside the CG iteration)",
                 "achieved": round(achieved, 1), "peak": peak, "unit": "GB/s", "frac": round(achieved / peak, 4),
                 "peak_source": peak_src, "traffic": load_traffic(prec) if dims == (64, 64, 64, 64) else None,
                 "algorithmic_bytes_per_launch": REALS_DSLASH_COMPULSORY * rsize * Vh,
                 "avg_launch_ms": round(ds_ms, 5), "launches_timed": n_ds,
-                "frac_of_theoretical_8184": round(achieved / THEORETICAL_HBM_GBS, 4)}
+                "frac_of_theoretical_8184": round(achieved / THEORETICAL_HBM_GBS, 4),
+                "read_stream_gbs": round(stream_gbs, 1), "frac_of_read_stream": round(achieved / stream_gbs, 4)}
     kernel_ms = {name: round(prof[k][1] / max(prof[k][0], 1), 5) for name, k in
                  (("dslash_oe", q.QCD_K_DSLASH), ("dslash_eo_epilogue_dot", q.QCD_K_DSLASH_EPI),
                   ("update_xr_norm", q.QCD_K_UPDATE_XR), ("update_p", q.QCD_K_UPDATE_P))}

@@ -215,6 +215,18 @@ qcd_status qcd_profile_read(qcd_ctx *ctx, int which, int *launches, double *tota
 long long qcd_launch_count(const qcd_ctx *ctx);
 
 /*
+ * Read-only streaming ceiling (measurement hook; a half-Dslash is 96 % reads,
+ * so its roofline is quoted against a read stream as well as against the copy peak and the
+ * theoretical peak).  Runs `reps` passes of a kernel that does nothing but load every 16 bytes of
+ * field f (any kind) once, with the Dslash's own link-load instruction (read-only path, no L1
+ * allocation, L2 evict_first), times them with CUDA events on the context stream, synchronises,
+ * and returns the average milliseconds per pass in *ms_per_pass (host pointer).
+ * GB/s = qcd_field_bytes(ctx, kind of f) / ms.  Use a field much larger than the 126 MB L2.
+ * Errors: QCD_EINVAL (NULL, foreign field, reps < 1), QCD_ECUDA.
+ */
+qcd_status qcd_stream_read(qcd_ctx *ctx, const qcd_field *f, int reps, double *ms_per_pass);
+
+/*
  * Tuning knob for the Dslash kernels (bench sweeps and A/B tests, Sec. 10):
  *   0 : the library's choice (128-thread blocks, 4 resident per SM for one vector; for several vectors
  *       the register kernel or the cp.async-staged kernel, whichever measured faster for that

@@ -33,7 +33,7 @@ SYMBOLS = [
     "qcd_field_download", "qcd_set_workspace", "qcd_dslash_eo", "qcd_dslash_oe", "qcd_apply_M",
     "qcd_cg_solve", "qcd_cg_begin", "qcd_cg_iterate", "qcd_cg_poll", "qcd_cg_finish",
     "qcd_cg_solve_host", "qcd_profile_enable", "qcd_profile_read", "qcd_launch_count",
-    "qcd_set_dslash_variant", "qcd_set_traversal_chunk", "qcd_set_cg_loop", "qcd_re_dot",
+    "qcd_set_dslash_variant", "qcd_set_traversal_chunk", "qcd_set_cg_loop", "qcd_re_dot", "qcd_stream_read",
     # variants and mixed precision
     "qcd_gauge_compress", "qcd_gauge_fix_temporal", "qcd_gauge_set_temporal_unit", "qcd_spinor_rotate",
     "qcd_workspace_bytes_multi", "qcd_dslash_eo_multi", "qcd_dslash_oe_multi", "qcd_cg_solve_multi",
@@ -99,6 +99,7 @@ def load_library() -> ctypes.CDLL:
         "qcd_set_traversal_chunk": (ci, [vp, ci]),
         "qcd_set_cg_loop": (ci, [vp, ci]),
         "qcd_re_dot": (ci, [vp, vp, vp, P(cd)]),
+        "qcd_stream_read": (ci, [vp, vp, ci, P(cd)]),
         "qcd_gauge_compress": (ci, [vp, vp, vp]),
         "qcd_gauge_fix_temporal": (ci, [vp, vp, vp, vp]),
         "qcd_gauge_set_temporal_unit": (ci, [vp, ci]),
@@ -302,6 +303,11 @@ class Context:
         r = ctypes.c_double()
         self._check(self.lib.qcd_re_dot(self.handle, a.handle, b.handle, ctypes.byref(r)), "qcd_re_dot")
         return r.value
+
+    def qcd_stream_read(self, f: Field, reps: int) -> float:
+        ms = ctypes.c_double()
+        self._check(self.lib.qcd_stream_read(self.handle, f.handle, int(reps), ctypes.byref(ms)), "qcd_stream_read")
+        return ms.value
 
     # ---- variants -------------------------------------------------------
     @staticmethod

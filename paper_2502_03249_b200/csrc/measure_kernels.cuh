@@ -1,0 +1,31 @@
+// Read-only streaming ceiling (SURVEY.md Sec. 7 "hard parts": a half-Dslash is 96 % reads, so
+// the denominator that says how close it is to what the memory system can deliver is a
+// kernel made of nothing but the Dslash's own link loads -- 16-byte, fully coalesced,
+// read-only path, no L1 allocation, L2 evict_first -- not a copy).  Measurement hook only:
+// it computes nothing the method needs.
+#pragma once
+#include "lattice.cuh"
+
+namespace qcd {
+
+enum { STREAM_BLOCK = 256, STREAM_LOADS = 8 };   // 8 independent 16-byte loads in flight per thread
+
+__global__ void __launch_bounds__(STREAM_BLOCK) stream_read_kernel(const double2 *__restrict__ p, size_t n16, double2 *sink)
+{
+    const uint64_t pol = l2_policy_evict_first();
+    const size_t base = (size_t)blockIdx.x * (STREAM_BLOCK * STREAM_LOADS) + threadIdx.x;
+    double2 v[STREAM_LOADS];
+#pragma unroll
+    for (int k = 0; k < STREAM_LOADS; ++k) {
+        const size_t i = base + (size_t)k * STREAM_BLOCK;
+        v[k] = i < n16 ? ld_stream(p + i, pol) : make_double2(0.0, 0.0);
+    }
+    unsigned long long x = 0;
+#pragma unroll
+    for (int k = 0; k < STREAM_LOADS; ++k)
+        x ^= (unsigned long long)__double_as_longlong(v[k].x) ^ (unsigned long long)__double_as_longlong(v[k].y);
+    // a NaN pattern no finite field carries in every word: keeps the loads alive, never stores
+    if (x == 0xfff7a5a5deadbeefULL) *sink = v[0];
+}
+
+} // namespace qcd

@@ -20,6 +20,7 @@
 #include "gauge_kernels.cuh"
 #include "lattice.cuh"
 #include "layout_kernels.cuh"
+#include "measure_kernels.cuh"
 #include "mixed_kernels.cuh"
 #include "reduce.cuh"
 
@@ -550,6 +551,36 @@ extern "C" qcd_status qcd_re_dot(qcd_ctx *ctx, const qcd_field *a, const qcd_fie
     CU(ctx, cudaMemcpyAsync(&ctx->h_scal[0], ctx->d_aux, sizeof(CgScalars), cudaMemcpyDeviceToHost, ctx->stream));
     CU(ctx, cudaStreamSynchronize(ctx->stream));
     *result = ctx->h_scal[0].dot;
+    return QCD_OK;
+}
+
+// Read-only streaming ceiling over a field's own bytes (measure_kernels.cuh): the denominator of
+// the Dslash roofline beside the copy peak and the theoretical peak.
+extern "C" qcd_status qcd_stream_read(qcd_ctx *ctx, const qcd_field *f, int reps, double *ms_per_pass)
+{
+    if (!ctx) return QCD_EINVAL;
+    if (!f || f->ctx != ctx || reps < 1 || !ms_per_pass) return fail(ctx, QCD_EINVAL, "qcd_stream_read: need a field of this context, reps >= 1 and a result pointer");
+    const size_t n16 = qcd_field_bytes(ctx, f->kind) / 16;
+    const size_t per = (size_t)STREAM_BLOCK * STREAM_LOADS;
+    const size_t grid = (n16 + per - 1) / per;
+    if (grid > 0x7fffffffULL) return fail(ctx, QCD_EINVAL, "qcd_stream_read: field too large for one launch");
+    cudaEvent_t e0, e1;
+    CU(ctx, cudaEventCreate(&e0));
+    CU(ctx, cudaEventCreate(&e1));
+    cudaError_t err = cudaEventRecord(e0, ctx->stream);
+    for (int r = 0; r < reps && err == cudaSuccess; ++r) {
+        LaunchScope ls(ctx, QCD_K_MISC);
+        stream_read_kernel<<<(unsigned)grid, STREAM_BLOCK, 0, ctx->stream>>>((const double2 *)f->ptr, n16, (double2 *)ctx->d_stage);
+        err = cudaGetLastError();
+    }
+    if (err == cudaSuccess) err = cudaEventRecord(e1, ctx->stream);
+    if (err == cudaSuccess) err = cudaEventSynchronize(e1);
+    float ms = 0.f;
+    if (err == cudaSuccess) err = cudaEventElapsedTime(&ms, e0, e1);
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    if (err != cudaSuccess) return fail(ctx, QCD_ECUDA, "qcd_stream_read: %s", cudaGetErrorString(err));
+    *ms_per_pass = (double)ms / reps;
     return QCD_OK;
 }
 

@@ -318,3 +318,30 @@ def test_cg_edge_cases(q):
     ctx.close()
     with pytest.raises(q.QcdError):
         q.Context((4, 4, 5, 4), 64)
+
+
+# ------------------------------------------------------------------------------------------
+# measurement hook
+# ------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("prec", [64, 32])
+def test_stream_read_hook(q, prec):
+    """qcd_stream_read times a read-only pass over a field (bench.py's third roofline denominator): it must
+    run on every field kind, including a ragged tail (4^4 gauge = 9216 sixteen-byte words fp32, not a
+    multiple of the 2048 one block reads), leave the field untouched, and reject bad arguments."""
+    dims = (4, 4, 4, 4)
+    ctx = q.Context(dims, prec)
+    U = qcd_inputs.gauge_field(dims, "haar", seed=3).astype(ctx.cdtype)
+    fU = ctx.field(q.QCD_GAUGE).upload(U)
+    fe = ctx.field(q.QCD_SPINOR_EVEN).upload(qcd_inputs.gaussian_source(dims, seed=1, parity=0).astype(ctx.cdtype))
+    n0 = ctx.qcd_launch_count()
+    assert ctx.qcd_stream_read(fU, 3) > 0.0
+    assert ctx.qcd_stream_read(fe, 1) > 0.0
+    assert ctx.qcd_launch_count() - n0 == 4
+    assert np.array_equal(fU.download(), U)
+    with pytest.raises(q.QcdError):
+        ctx.qcd_stream_read(fU, 0)
+    other = q.Context(dims, prec)
+    with pytest.raises(q.QcdError):
+        other.qcd_stream_read(fU, 1)
+    other.close()
+    ctx.close()
