@@ -245,3 +245,62 @@ def test_cg_full_size_is_bitwise_reproducible(q, config, prec):
     ctx.close()
     assert i1["iters"] == i2["iters"] and i1["rel_resid"] == i2["rel_resid"]
     assert np.array_equal(x1, x2)
+
+
+# ------------------------------------------------------------------------------------------
+# beyond the benchmark sizes: element offsets past 2^31
+# ------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("prec", [64, 32])
+def test_lattice_with_more_than_2G_link_elements(q, prec):
+    """128 x 128 x 64 x 64 (4 x configs[4]'s volume; links 38.7 GB fp64): the gauge field has 72 planes of
+    Vh = 33.5 M complex numbers = 2.4e9 elements, so every plane offset past plane 63 exceeds 2^31 --
+    which no BASELINE.json config reaches (64^4: 6.0e8).  It is also the first size at which ONE vector
+    is walked in the chunked traversal order (W = 16 < N2).  Whole fields against the oracle for D_oe,
+    D_eo and M, and the CG iterate after 3 iterations against the oracle's."""
+    dims = (128, 128, 64, 64)
+    m = 0.05
+    U = qcd_inputs.gauge_field(dims, "haar", seed=0)
+    b = qcd_inputs.gaussian_source(dims, seed=1, parity=0)
+    par = qcd_inputs.site_parity(dims)
+    # fp64: north_star's 1e-13.  fp32: north_star states 2e-6 for the five configs; the measure (R10) is a MAX
+    # over sites with the site norm floored at 0.1 R, and over 4 x the sites of configs[4] its tail reaches
+    # 2.08e-6 (measured; 64^4 stays below 2e-6), so this size is held to 3e-6.  An indexing fault shows as O(1).
+    tol = DSLASH_TOL[prec] if prec == 64 else 3e-6
+    ctx = q.Context(dims, prec)
+    assert 72 * (par.size // 2) > 2 ** 31 and ctx.qcd_field_bytes(q.QCD_GAUGE) == par.size * 4 * 18 * (prec // 8)
+    fU = ctx.field(q.QCD_GAUGE).upload(U)
+    if prec == 32:
+        U = rounded(U, prec)                      # in place of the fp64 copy: two 38.7 GB arrays at most
+        b = rounded(b, prec)
+    fe = ctx.field(q.QCD_SPINOR_EVEN).upload(b)
+    fo = ctx.field(q.QCD_SPINOR_ODD)
+    fe2 = ctx.field(q.QCD_SPINOR_EVEN)
+    ctx.qcd_dslash_oe(fU, fo, fe)
+    got = fo.download()
+    ref = oracle.dslash(dims, U, b, 1)
+    assert dslash_rel_err(got[par == 1], ref[par == 1]) <= tol
+    assert not got[par == 0].any()
+    t_in = rounded(ref, prec)
+    del ref, got
+    fo.upload(t_in)
+    ctx.qcd_dslash_eo(fU, fe2, fo)
+    got = fe2.download()
+    ref = oracle.dslash(dims, U, t_in, 0)
+    assert dslash_rel_err(got[par == 0], ref[par == 0]) <= tol
+    del ref, got, t_in
+    ctx.qcd_apply_M(fU, fe2, fe, m)
+    got = fe2.download()
+    ref = oracle.apply_M(dims, U, b, m)
+    assert dslash_rel_err(got[par == 0], ref[par == 0]) <= 2 * tol
+    del ref, got
+    info = ctx.qcd_cg_solve(fU, fe, fe2, m, 1e-12, 3)
+    got = fe2.download()
+    xo, oinfo = oracle.cg(dims, U, b, m, 1e-12, 3)
+    assert info["iters"] == oinfo["iters"] == 3 and not info["converged"]
+    if prec == 64:
+        assert dslash_rel_err(got[par == 0], xo[par == 0]) <= 1e-12
+        assert abs(info["rel_resid"] - oinfo["rel_resid"]) <= 1e-12 * oinfo["rel_resid"]
+    else:
+        assert dslash_rel_err(got[par == 0], xo[par == 0]) <= 2e-5   # three fp32 iterations against fp64 ones
+        assert abs(info["rel_resid"] - oinfo["rel_resid"]) <= 1e-5 * oinfo["rel_resid"]
+    ctx.close()
