@@ -579,7 +579,7 @@ def extras(args, q, torch, ctx, out, cfg, dims, U, b, fU, fb, fx, fo, peak):
                       "ms_per_iter": round(1e3 * info["seconds"] / max(info["iters"], 1), 5),
                       "rel_resid_recurrence": info["rel_resid"], "true_resid_oracle_fp64": true64}
     # CPU baseline: the oracle as it stands, a bounded sample of the same workload
-    nit = 3
+    nit = 12                                                # ~10 s of oracle time at 64^4 on 16 cores
     t0 = time.time()
     _, oinfo = oracle.cg(dims, U, b, m, 1e-300, nit)
     t_or = time.time() - t0
