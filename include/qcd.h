@@ -190,6 +190,21 @@ qcd_status qcd_cg_poll(qcd_ctx *ctx, int *state, int *iters, double *rel_resid);
 qcd_status qcd_cg_finish(qcd_ctx *ctx, qcd_cg_info *info);
 
 /*
+ * Residual history of the most recent solve of this context (SURVEY.md Sec. 5 "metrics"):
+ * host_out[j] = <r,r> / <b,b> after j + 1 M applications, j = 0 .. iters-1 -- the squared relative
+ * recurrence residual CG tests against tol^2 (reading R6).  Recorded on the device by the kernel
+ * that advances the recurrence (no extra launch or host round trip during the solve), for the
+ * first 16384 iterations of every right-hand side; all three solver loops record it.
+ *   rhs      : 0 for qcd_cg_solve; 0 .. n-1 after a multi solve
+ *   host_out : HOST array of `cap` doubles (may be NULL when cap = 0)
+ *   n        : receives min(iters, cap, 16384)
+ * Valid from qcd_cg_finish / the return of qcd_cg_solve until the next solve begins on the context
+ * (the inner solves of qcd_cg_solve_mixed overwrite the fp32 context's history).  Synchronises.
+ * Errors: QCD_EINVAL (bad argument, solve in progress), QCD_ECUDA.
+ */
+qcd_status qcd_cg_history(qcd_ctx *ctx, int rhs, double *host_out, int cap, int *n);
+
+/*
  * qcd_cg_solve with HOST source and solution in the canonical spinor layout (full-lattice
  * arrays, even sites used): upload b, solve, download x.  b_dev / x_dev are the device
  * fields used for staging.  info->seconds covers copies and solve.

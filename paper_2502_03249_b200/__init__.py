@@ -33,7 +33,7 @@ SYMBOLS = [
     "qcd_field_download", "qcd_set_workspace", "qcd_dslash_eo", "qcd_dslash_oe", "qcd_apply_M",
     "qcd_cg_solve", "qcd_cg_begin", "qcd_cg_iterate", "qcd_cg_poll", "qcd_cg_finish",
     "qcd_cg_solve_host", "qcd_profile_enable", "qcd_profile_read", "qcd_launch_count",
-    "qcd_set_dslash_variant", "qcd_set_traversal_chunk", "qcd_set_cg_loop", "qcd_re_dot", "qcd_stream_read",
+    "qcd_set_dslash_variant", "qcd_set_traversal_chunk", "qcd_set_cg_loop", "qcd_re_dot", "qcd_stream_read", "qcd_cg_history",
     # variants and mixed precision
     "qcd_gauge_compress", "qcd_gauge_fix_temporal", "qcd_gauge_set_temporal_unit", "qcd_spinor_rotate",
     "qcd_workspace_bytes_multi", "qcd_dslash_eo_multi", "qcd_dslash_oe_multi", "qcd_cg_solve_multi",
@@ -100,6 +100,7 @@ def load_library() -> ctypes.CDLL:
         "qcd_set_cg_loop": (ci, [vp, ci]),
         "qcd_re_dot": (ci, [vp, vp, vp, P(cd)]),
         "qcd_stream_read": (ci, [vp, vp, ci, P(cd)]),
+        "qcd_cg_history": (ci, [vp, ci, P(cd), ci, P(ci)]),
         "qcd_gauge_compress": (ci, [vp, vp, vp]),
         "qcd_gauge_fix_temporal": (ci, [vp, vp, vp, vp]),
         "qcd_gauge_set_temporal_unit": (ci, [vp, ci]),
@@ -278,6 +279,15 @@ class Context:
                                                     float(m), float(tol), int(maxiter), ctypes.byref(i)),
                          "qcd_cg_solve_host", self._CG_OK)
         return self._info(i, st)
+
+    def qcd_cg_history(self, rhs: int = 0, cap: int = 16384) -> np.ndarray:
+        """rr_k / bb after k = 1 .. iters M applications of the most recent solve (numpy float64)."""
+        out = np.zeros(int(cap), dtype=np.float64)
+        n = ctypes.c_int()
+        self._check(self.lib.qcd_cg_history(self.handle, int(rhs), out.ctypes.data_as(ctypes.POINTER(ctypes.c_double)), int(cap),
+                                                 ctypes.byref(n)),
+                    "qcd_cg_history")
+        return out[: n.value].copy()
 
     def qcd_profile_enable(self, on: bool):
         self._check(self.lib.qcd_profile_enable(self.handle, 1 if on else 0), "qcd_profile_enable")

@@ -145,6 +145,7 @@ __global__ void __launch_bounds__(BLAS_BLOCK) cg_update_xr_kernel(
             scal->rr = rr_new;
             const int k = scal->k + 1;
             scal->k = k;
+            if (scal->hist && k <= scal->hist_cap) scal->hist[k - 1] = rr_new;
             if (rr_new != rr_new) scal->flag = 3;
             else if (rr_new <= scal->tol2bb) scal->flag = 1;
             else if (k >= scal->maxiter) scal->flag = 2;

@@ -184,6 +184,10 @@ __global__ void __launch_bounds__(PERSIST_BLOCK, 3) cg_persistent_kernel(const P
         beta = rr_new / rr;
         rr = rr_new;
         k += 1;
+        if (gtid == 0) {                                           // residual history (qcd_cg_history)
+            double *const hist = a.scal->hist;
+            if (hist && k <= a.scal->hist_cap) hist[k - 1] = rr_new;
+        }
         if (rr_new != rr_new) flag = 3;
         else if (rr_new <= tol2bb) flag = 1;
         else if (k >= maxiter) flag = 2;

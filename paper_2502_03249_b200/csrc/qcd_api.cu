@@ -29,7 +29,7 @@ using namespace qcd;
 // ------------------------------------------------------------------------------------------
 // context
 // ------------------------------------------------------------------------------------------
-enum { PROF_MAX = 4096, STAGE_BYTES = 32 << 20, POLL_SLOTS = 2 };
+enum { PROF_MAX = 4096, STAGE_BYTES = 32 << 20, POLL_SLOTS = 2, HIST_CAP = 16384 };
 
 struct qcd_field {
     qcd_ctx *ctx;
@@ -60,6 +60,7 @@ struct qcd_ctx {
     CgScalars *d_aux;         // scratch state for qcd_apply_M / qcd_re_dot / the mixed solver
     double *d_partials;       // stage-1 partial sums
     unsigned *d_tickets;      // first-level tickets of the two-level last-block election (reduce.cuh)
+    double *d_hist;           // residual history, MAXRHS x HIST_CAP (qcd_cg_history)
     int partials_cap;
     CgScalars *h_scal;        // pinned, POLL_SLOTS x MAXRHS entries
     cudaEvent_t poll_ev[POLL_SLOTS];
@@ -180,6 +181,7 @@ extern "C" qcd_status qcd_init(qcd_ctx **out, const int dims[4], int precision, 
     c->ws = nullptr; c->ws_bytes = 0;
     memset(&c->cg, 0, sizeof c->cg);
     c->d_scal = c->d_aux = nullptr; c->d_partials = nullptr; c->d_tickets = nullptr; c->h_scal = nullptr; c->d_stage = nullptr;
+    c->d_hist = nullptr;
     for (int i = 0; i < POLL_SLOTS; ++i) c->poll_ev[i] = nullptr;
 
     c->partials_cap = MAXRHS * (dslash_grid_max(c) > blas_grid(c) ? dslash_grid_max(c) : blas_grid(c));
@@ -193,6 +195,13 @@ extern "C" qcd_status qcd_init(qcd_ctx **out, const int dims[4], int precision, 
     for (int i = 0; i <= MAXRHS && err == cudaSuccess; ++i) {
         unsigned *l1 = c->d_tickets + (size_t)i * groups;
         err = cudaMemcpy(&c->d_scal[i].l1, &l1, sizeof l1, cudaMemcpyHostToDevice);
+    }
+    if (err == cudaSuccess) err = cudaMalloc(&c->d_hist, (size_t)MAXRHS * HIST_CAP * sizeof(double));
+    for (int i = 0; i < MAXRHS && err == cudaSuccess; ++i) {          // d_aux (entry MAXRHS) keeps hist = NULL
+        double *h = c->d_hist + (size_t)i * HIST_CAP;
+        const int cap = HIST_CAP;
+        err = cudaMemcpy(&c->d_scal[i].hist, &h, sizeof h, cudaMemcpyHostToDevice);
+        if (err == cudaSuccess) err = cudaMemcpy(&c->d_scal[i].hist_cap, &cap, sizeof cap, cudaMemcpyHostToDevice);
     }
     if (err == cudaSuccess) err = cudaMalloc(&c->d_stage, STAGE_BYTES);
     if (err == cudaSuccess) err = cudaMallocHost(&c->h_scal, POLL_SLOTS * MAXRHS * sizeof(CgScalars));
@@ -220,6 +229,7 @@ extern "C" qcd_status qcd_finalize(qcd_ctx *c)
     if (c->d_scal) cudaFree(c->d_scal);
     if (c->d_partials) cudaFree(c->d_partials);
     if (c->d_tickets) cudaFree(c->d_tickets);
+    if (c->d_hist) cudaFree(c->d_hist);
     if (c->d_stage) cudaFree(c->d_stage);
     if (c->h_scal) cudaFreeHost(c->h_scal);
     delete c;
@@ -746,6 +756,28 @@ extern "C" qcd_status qcd_cg_finish_multi(qcd_ctx *ctx, qcd_cg_info *info)
     }
     if (res == QCD_EBREAKDOWN) return fail(ctx, res, "qcd_cg: breakdown (<p,Mp> <= 0 or NaN)");
     if (res == QCD_ENOTCONVERGED) return fail(ctx, res, "qcd_cg: not converged");
+    return QCD_OK;
+}
+
+// Residual history of the most recent solve (recorded on the device by the kernel that advances the
+// recurrence; no extra launch, no host round trip during the solve).
+extern "C" qcd_status qcd_cg_history(qcd_ctx *ctx, int rhs, double *host_out, int cap, int *n)
+{
+    if (!ctx) return QCD_EINVAL;
+    if (rhs < 0 || rhs >= MAXRHS || cap < 0 || (cap > 0 && !host_out) || !n) return fail(ctx, QCD_EINVAL, "qcd_cg_history: bad argument");
+    if (ctx->cg.active) return fail(ctx, QCD_EINVAL, "qcd_cg_history: a solve is in progress (qcd_cg_finish first)");
+    CgScalars s;
+    CU(ctx, cudaMemcpyAsync(&ctx->h_scal[0], ctx->d_scal + rhs, sizeof(CgScalars), cudaMemcpyDeviceToHost, ctx->stream));
+    CU(ctx, cudaStreamSynchronize(ctx->stream));
+    s = ctx->h_scal[0];
+    int m = s.k < HIST_CAP ? s.k : HIST_CAP;
+    if (m > cap) m = cap;
+    if (m > 0) {
+        CU(ctx, cudaMemcpyAsync(host_out, ctx->d_hist + (size_t)rhs * HIST_CAP, (size_t)m * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+        CU(ctx, cudaStreamSynchronize(ctx->stream));
+        for (int j = 0; j < m; ++j) host_out[j] /= s.bb;
+    }
+    *n = m;
     return QCD_OK;
 }
 

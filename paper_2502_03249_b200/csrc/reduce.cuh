@@ -30,6 +30,8 @@ struct CgScalars {
     int flag;         // 0 running, 1 converged, 2 maxiter reached, 3 breakdown
     unsigned ticket;  // top-level last-block ticket, wraps to 0 by itself (atomicInc)
     unsigned *l1;     // first-level tickets, one per group of TICKET_GROUP blocks (set once by qcd_init)
+    double *hist;     // residual history: hist[j] = <r,r> after j + 1 M applications, j < hist_cap (set once by qcd_init; may be NULL)
+    int hist_cap;
 };
 
 __device__ __forceinline__ double warp_sum(double v)

@@ -345,3 +345,75 @@ def test_stream_read_hook(q, prec):
         other.qcd_stream_read(fU, 1)
     other.close()
     ctx.close()
+
+
+# ------------------------------------------------------------------------------------------
+# residual history: the recurrence, iteration by iteration, against the oracle's
+# ------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("prec", [64, 32])
+@pytest.mark.parametrize("loop", [1, 2, 3])
+def test_cg_residual_history_matches_oracle(q, loop, prec):
+    """configs[1].  qcd_cg_history returns rr_k / bb after every M application, recorded on the device.  The
+    oracle records the same sequence (oracle_cg `history`).  Equal alpha_k, beta_k up to rounding means the
+    two sequences agree entry by entry -- a far finer check of the recurrence than the iteration count: a
+    wrong beta, a stale alpha or a dot product over the wrong sites shows at the first entries.  All three
+    solver loops (kernel by kernel, graph replay, persistent kernel) must record it."""
+    import torch
+    cfg, U, b = qcd_inputs.config_inputs(1)
+    dims, m = cfg["dims"], cfg["m"]
+    tol = cfg["tol64"] if prec == 64 else cfg["tol32"]
+    cd = np.complex128 if prec == 64 else np.complex64
+    _, oinfo = oracle.cg(dims, U.astype(cd), b.astype(cd), m, tol, cfg["maxiter"], history=True)
+    ho = oinfo["history"]
+    with torch.cuda.stream(torch.cuda.Stream()):                    # graph replay needs a non-default stream
+        ctx = q.Context(dims, prec)
+        ctx.qcd_set_cg_loop(loop)
+        fU = ctx.field(q.QCD_GAUGE).upload(U)
+        fb, fx = ctx.field(q.QCD_SPINOR_EVEN).upload(b), ctx.field(q.QCD_SPINOR_EVEN)
+        info = ctx.qcd_cg_solve(fU, fb, fx, m, tol, cfg["maxiter"])
+        h = ctx.qcd_cg_history()
+        assert info["converged"] and len(h) == info["iters"]
+        assert h[-1] == info["rel_resid"] ** 2 or abs(np.sqrt(h[-1]) - info["rel_resid"]) <= 1e-15 * info["rel_resid"]
+        assert np.all(h[:-1] > tol * tol) and h[-1] <= tol * tol    # stopped at the FIRST iteration below tol
+        n = min(len(h), len(ho))
+        assert abs(len(h) - len(ho)) <= 2
+        rel = np.abs(h[:n] - ho[:n]) / ho[:n]
+        if prec == 64:
+            assert rel[:10].max() <= 1e-12 and rel.max() <= 1e-7, (rel[:10].max(), rel.max())
+        else:
+            assert rel[:10].max() <= 2e-5 and rel[: n - 2].max() <= 5e-2, (rel[:10].max(), rel.max())
+        # cap smaller than the solve, and the argument checks
+        assert np.array_equal(ctx.qcd_cg_history(0, 5), h[:5])
+        assert len(ctx.qcd_cg_history(0, 0)) == 0
+        with pytest.raises(q.QcdError):
+            ctx.qcd_cg_history(q.QCD_MAX_RHS, 4)
+        # a solve stopped at maxiter records exactly maxiter entries, equal to the first ones of the full solve
+        info7 = ctx.qcd_cg_solve(fU, fb, fx, m, tol, 7)
+        h7 = ctx.qcd_cg_history()
+        assert info7["iters"] == 7 and len(h7) == 7
+        assert np.allclose(h7, h[:7], rtol=1e-12 if prec == 64 else 1e-5, atol=0)
+        ctx.close()
+
+
+def test_cg_history_multi_rhs(q):
+    """Lock-step solve of 3 right-hand sides: each keeps its own history, equal to its single solve's."""
+    dims, m, tol = (8, 8, 8, 8), 0.1, 1e-10
+    U = qcd_inputs.gauge_field(dims, "haar", seed=0)
+    srcs = [qcd_inputs.gaussian_source(dims, seed=s_) for s_ in (1, 2, 3)]
+    srcs[1] = srcs[1] * 0.0                                          # a zero source stops at iteration 0
+    ctx = q.Context(dims, 64, nrhs=3)
+    ctx.qcd_set_cg_loop(1)
+    fU = ctx.field(q.QCD_GAUGE).upload(U)
+    fb = [ctx.field(q.QCD_SPINOR_EVEN).upload(s_) for s_ in srcs]
+    fx = [ctx.field(q.QCD_SPINOR_EVEN) for _ in srcs]
+    single = []
+    for i in range(3):
+        ctx.qcd_cg_solve(fU, fb[i], fx[i], m, tol, 5000)
+        single.append(ctx.qcd_cg_history())
+    infos = ctx.qcd_cg_solve_multi(fU, fb, fx, m, tol, 5000)
+    for i in range(3):
+        h = ctx.qcd_cg_history(i)
+        assert len(h) == infos[i]["iters"] == len(single[i])
+        assert np.array_equal(h, single[i])                          # identical arithmetic and reduction order
+    assert len(single[1]) == 0
+    ctx.close()
