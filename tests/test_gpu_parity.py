@@ -417,3 +417,52 @@ def test_cg_history_multi_rhs(q):
         assert np.array_equal(h, single[i])                          # identical arithmetic and reduction order
     assert len(single[1]) == 0
     ctx.close()
+
+
+# ------------------------------------------------------------------------------------------
+# degenerate cases of the method: breakdown, massless operator
+# ------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("loop", [1, 3])
+def test_cg_breakdown_on_nan(q, loop):
+    """DESIGN.md R19: <p,Mp> <= 0 or NaN ends the solve with QCD_EBREAKDOWN (M is positive definite for m > 0,
+    so only non-finite data can get there).  A NaN in the source is caught before the first M application, a
+    NaN in the links at the first <p,Mp>; the oracle reports breakdown at the same iteration (0)."""
+    dims = (8, 8, 8, 8)
+    U = qcd_inputs.gauge_field(dims, "haar", seed=0)
+    b = qcd_inputs.gaussian_source(dims, seed=1)
+    ctx = q.Context(dims, 64)
+    ctx.qcd_set_cg_loop(loop)
+    fU = ctx.field(q.QCD_GAUGE).upload(U)
+    fx = ctx.field(q.QCD_SPINOR_EVEN)
+    bn = b.copy()
+    bn[0, 1] = np.nan                                               # site 0 is even
+    fb = ctx.field(q.QCD_SPINOR_EVEN).upload(bn)
+    info = ctx.qcd_cg_solve(fU, fb, fx, 0.1, 1e-10, 100)
+    _, oinfo = oracle.cg(dims, U, bn, 0.1, 1e-10, 100)
+    assert info["status"] == q.QCD_EBREAKDOWN and not info["converged"] and info["iters"] == 0
+    assert oinfo["status"] == 5 and oinfo["iters"] == 0             # the oracle's own code for breakdown
+    Un = U.copy()
+    Un[37, 2, 1, 1] = np.nan
+    fU.upload(Un)
+    fb.upload(b)
+    info = ctx.qcd_cg_solve(fU, fb, fx, 0.1, 1e-10, 100)
+    _, oinfo = oracle.cg(dims, Un, b, 0.1, 1e-10, 100)
+    assert info["status"] == q.QCD_EBREAKDOWN and info["iters"] == 0, info
+    assert oinfo["status"] == 5 and oinfo["iters"] == 0
+    # the context is usable afterwards
+    fU.upload(U)
+    info = ctx.qcd_cg_solve(fU, fb, fx, 0.1, 1e-10, 2000)
+    assert info["status"] == q.QCD_OK and oracle.true_residual(dims, U, b, fx.download(), 0.1) <= 1e-10
+    ctx.close()
+
+
+def test_cg_massless(q):
+    """m = 0 is allowed (R19): M = -D_eo D_oe = D_oe^dagger D_oe is still positive definite on Haar links at 4^4
+    (lambda_min ~ 3e-5), only badly conditioned.  Same checks as at m > 0."""
+    cfg, U, b = qcd_inputs.config_inputs(0)
+    dims, tol = cfg["dims"], 1e-8
+    x, info = _solve(q, dims, 64, U, b, 0.0, tol, 20000)
+    xo, oinfo = oracle.cg(dims, U, b, 0.0, tol, 20000)
+    assert info["converged"] and oinfo["converged"]
+    assert iters_close(info["iters"], oinfo["iters"]), (info["iters"], oinfo["iters"])
+    assert oracle.true_residual(dims, U, b, x, 0.0) <= tol * 1.01
