@@ -242,7 +242,13 @@ def variants_sweep(q, torch, ctx, fU_full, dims, peak, nmulti=(1, 2, 3, 4, 6, 8)
             rows.append({"links": name, "nmulti": n, "ms": round(ms, 5),
                          "tflops": round(FLOP_PER_SITE * n * Vh / ms / 1e9, 3),
                          "gbs_compulsory": round(gbs, 1), "frac_of_measured_copy_peak": round(gbs / peak, 4),
-                         "ai_nominal_flop_per_byte": round(FLOP_PER_SITE * n / (nom * rsize), 3)})
+                         "ai_nominal_flop_per_byte": round(FLOP_PER_SITE * n / (nom * rsize), 3),
+                         # Eq. (2) of the paper: attainable = min(peak, AI x bandwidth); the
+                         # bandwidth term binds at every n here.  With the paper's NOMINAL bytes (no cache reuse
+                         # of the neighbour vectors) a kernel whose L2 serves that reuse lands ABOVE this line,
+                         # as the paper observes on A100; with compulsory bytes it cannot.
+                         "eq2_attainable_tflops_nominal_ai": round(FLOP_PER_SITE * n / (nom * rsize) * peak / 1e3, 3),
+                         "eq2_attainable_tflops_compulsory_ai": round(FLOP_PER_SITE * n / (comp * rsize) * peak / 1e3, 3)})
         ctx.qcd_gauge_set_temporal_unit(fU, False)
     for f in fins + fouts + [f12]:
         f.free()
