@@ -26,6 +26,22 @@ template <> struct DslashCfg<float, 6> { enum { BLOCK = 128, MINB = 3 }; };
 template <> struct DslashCfg<float, 7> { enum { BLOCK = 128, MINB = 2 }; };
 template <> struct DslashCfg<float, 8> { enum { BLOCK = 128, MINB = 2 }; };
 
+// Temporal-gauge kernels for one vector (TG = 1, NRHS = 1) move 27-55 % fewer bytes per site with the
+// same index arithmetic, run below the DRAM limit and are sensitive to how many warps are resident
+// and to how far ptxas hoists loads under the register cap.  Occupancy sweep at 64^4 fp64 (MINB = 2 ... 8,
+// DESIGN.md Sec. 10 "Occupancy of the temporal-gauge kernels"):
+//   * MODE 2 (D_eo + epilogue + dot) wants 6 blocks (80 registers, 24 warps; the chunk loop makes ptxas
+//     fill a 128-register cap without putting more loads in flight): two-row 1.11 -> 0.96 ms, full 1.58 -> 1.34;
+//   * MODE 0 / 1 on full links want 3 blocks (168-register cap: the loads of the next direction are
+//     hoisted over the current one's FMAs): 1.44 -> 1.17-1.20 ms; on two-row links 4 blocks stay best.
+// fp32 kernels keep 4 blocks everywhere (their registers hold twice the loads already).
+template <typename T, int MODE, int NROW, int TG, int NRHS>
+struct DslashTune {
+    enum { BLOCK = DslashCfg<T, NRHS>::BLOCK,
+           MINB = (sizeof(T) == 8 && TG == 1 && NRHS == 1) ? (MODE == 2 ? 6 : (NROW == 3 ? 3 : DslashCfg<T, NRHS>::MINB))
+                                                            : DslashCfg<T, NRHS>::MINB };
+};
+
 // Kernels that end with a block reduction (MODE 2) walk several chunks of BLOCK sites per block so
 // that the ~2 us reduction tail is paid once per several hundred sites, not by every 128: the grid
 // is sized to about REDUCE_GRID blocks (32 waves of 148 SMs x 4 resident blocks; 4 chunks per block
@@ -100,7 +116,7 @@ static cudaError_t launch_nrhs(const DslashLaunch &d)
         default: break;
         }
     }
-    return launch_cfg<T, MODE, NROW, TG, NRHS, DslashCfg<T, NRHS>::BLOCK, DslashCfg<T, NRHS>::MINB>(d);
+    return launch_cfg<T, MODE, NROW, TG, NRHS, DslashTune<T, MODE, NROW, TG, NRHS>::BLOCK, DslashTune<T, MODE, NROW, TG, NRHS>::MINB>(d);
 }
 
 template <typename T, int MODE, int NROW, int TG>
