@@ -255,7 +255,7 @@ __global__ void __launch_bounds__(BLOCK, MINB) dslash_kernel(const DslashArgs<T,
             } else if (NRHS <= 2 && sizeof(T) == 4) {
                 // temporal gauge, mu = 3, fp32: both neighbour vectors are requested before anything is
                 // consumed; the two links are needed on one time slice each only (warp-uniform branches).
-                // Measured at 64^4: fp32 two-row D_oe 0.45 -> 0.427 ms, D_eo + epilogue + dot 0.605 -> 0.565;
+                // Measured at 64^4 (burst timings): fp32 two-row D_oe 0.45 -> 0.427 ms, D_eo + epilogue + dot 0.605 -> 0.565;
                 // in fp64 the same code is slower at the 128-register cap (0.85 -> 0.92 ms), so fp64 keeps
                 // the hop-by-hop form below.
                 C pf[NRHS][3], pb[NRHS][3], uf[9], ub[9];
