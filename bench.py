@@ -98,7 +98,7 @@ class ClockSampler:
     """Samples SM clock and throttle reasons through NVML while the timed region runs."""
 
     def __init__(self, index: int):
-        self.samples, self.reasons, self.max_mhz = [], set(), None
+        self.samples, self.reasons, self.max_mhz, self.power = [], set(), None, []
         self._stop = threading.Event()
         self._thr = None
         try:
@@ -129,6 +129,7 @@ class ClockSampler:
                 for k, bit in names.items():
                     if r & bit:
                         self.reasons.add(k)
+                self.power.append(nv.nvmlDeviceGetPowerUsage(self.h) / 1e3)
             except Exception:
                 pass
             time.sleep(0.01)
@@ -148,7 +149,8 @@ class ClockSampler:
         if not self.samples:
             return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons), "samples": 0}
         return {"sm_mhz": float(np.median(self.samples)), "sm_max_mhz": self.max_mhz,
-                "reasons": sorted(self.reasons), "samples": len(self.samples)}
+                "reasons": sorted(self.reasons), "samples": len(self.samples),
+                "power_w": round(float(np.median(self.power)), 1) if self.power else None}
 
 
 # ---- multi-rank plumbing ---------------------------------------------------------------------
@@ -332,9 +334,10 @@ FLOP_PER_CG_ITER = 2 * FLOP_PER_SITE + 72     # per even site: two half-Dslash +
 
 
 def size_sweep_report(q, torch, device, sizes=((8, 8, 8, 8), (12, 12, 12, 12), (16, 16, 16, 16), (24, 24, 24, 24),
-                                               (32, 32, 32, 32), (48, 48, 48, 12)), iters=200):
+                                               (32, 32, 32, 32), (48, 48, 48, 12), (32, 32, 64, 64)), iters=200):
     """The paper's Fig. 3 experiment: Dslash and CG throughput against the lattice size, in
-    single and double precision (the 64^4 point is the headline above).  Dslash: 20 back-to-back D_oe launches;
+    single and double precision (the 64^4 point is the headline above; 32^2 x 64^2 is the size beyond which the
+    paper's MI250X curve degrades, PAPER.md:54).  Dslash: 20 back-to-back D_oe launches;
     CG: qcd_cg_solve with an unreachable tolerance and maxiter = `iters`, i.e. the solver loop the library picks
     for that size (persistent kernel while the lattice fits the L2, kernel-by-kernel beyond).  GFLOP/s with
     570 flop per site (Dslash) and 2 x 570 + 72 flop per even site and iteration (CG)."""
