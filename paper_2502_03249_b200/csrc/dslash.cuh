@@ -134,28 +134,44 @@ __device__ __forceinline__ void vec_acc(C acc[3], const C p[3])
 }
 
 // out = acc (MODE 0) or m^2 v - acc (MODE >= 1); MODE 2 also accumulates Re<v,out> per vector.
+// The 3 NRHS loads of v(x) are all issued before the first store: written as load / FMA / store per
+// component, every load after the first has to wait behind the preceding store (the compiler cannot
+// prove that out does not alias v), which exposes 3 NRHS memory round trips at the end of every thread
+// -- measured as +1.0 ms on the four-vector kernel (3.2 instead of 2.2 ms without the loads).  v(x) is
+// read once, so it is streamed like a link (read-only path, no L1 allocation, evict_first).
 template <typename T, int MODE, int NRHS>
 __device__ __forceinline__ void dslash_epilogue(const DslashArgs<T, NRHS> &a, int cb, typename Cplx<T>::type (&acc)[NRHS][3],
-                                                double (&dot)[NRHS])
+                                                double (&dot)[NRHS], uint64_t pol_stream)
 {
     typedef typename Cplx<T>::type C;
     const size_t Vh = (size_t)a.L.Vh;
+    if (MODE >= 1) {
+        C vv[NRHS][3];
 #pragma unroll
-    for (int r = 0; r < NRHS; ++r) {
-        if (MODE >= 1) {
+        for (int r = 0; r < NRHS; ++r)
 #pragma unroll
             for (int c = 0; c < 3; ++c) {
-                const C vv = a.v[r][(size_t)c * Vh + cb];
-                C o;
-                o.x = fma(a.m2, vv.x, -acc[r][c].x);
-                o.y = fma(a.m2, vv.y, -acc[r][c].y);
-                a.out[r][(size_t)c * Vh + cb] = o;
-                if (MODE == 2) dot[r] += (double)vv.x * (double)o.x + (double)vv.y * (double)o.y;
+                // one vector: the plain load (the L2 prefetch issued before the first hop has brought the line in;
+                // A/B at 64^4 is a wash in fp64 and the streamed form loses 8 % on the fp32 two-row temporal-gauge kernel)
+                if (NRHS == 1) vv[r][c] = a.v[r][(size_t)c * Vh + cb];
+                else vv[r][c] = ld_stream(a.v[r] + (size_t)c * Vh + cb, pol_stream);
             }
-        } else {
+#pragma unroll
+        for (int r = 0; r < NRHS; ++r) {
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+                C o;
+                o.x = fma(a.m2, vv[r][c].x, -acc[r][c].x);
+                o.y = fma(a.m2, vv[r][c].y, -acc[r][c].y);
+                a.out[r][(size_t)c * Vh + cb] = o;
+                if (MODE == 2) dot[r] += (double)vv[r][c].x * (double)o.x + (double)vv[r][c].y * (double)o.y;
+            }
+        }
+    } else {
+#pragma unroll
+        for (int r = 0; r < NRHS; ++r)
 #pragma unroll
             for (int c = 0; c < 3; ++c) a.out[r][(size_t)c * Vh + cb] = acc[r][c];
-        }
     }
 }
 
@@ -314,7 +330,7 @@ __global__ void __launch_bounds__(BLOCK, MINB) dslash_kernel(const DslashArgs<T,
             }
         }
 
-        dslash_epilogue<T, MODE, NRHS>(a, cb, acc, dot);
+        dslash_epilogue<T, MODE, NRHS>(a, cb, acc, dot, pol_stream);
     }
     }
     dslash_reduce<T, MODE, NRHS, BLOCK>(a, dot);
@@ -425,7 +441,7 @@ __global__ void __launch_bounds__(BLOCK, MINB) dslash_staged_kernel(const Dslash
             }
             if (h + DEPTH < 8) issue(h + DEPTH);
         }
-        dslash_epilogue<T, MODE, NRHS>(a, cb, acc, dot);
+        dslash_epilogue<T, MODE, NRHS>(a, cb, acc, dot, pol_stream);
     }
     }
     dslash_reduce<T, MODE, NRHS, BLOCK>(a, dot);
