@@ -130,13 +130,19 @@ __global__ void __launch_bounds__(PERSIST_BLOCK, 3) cg_persistent_kernel(const P
         for (int cb = gtid; cb < Vh; cb += gthreads) {
             C acc[3];
             persistent_site<T, NROW, TG, true>(acc, a.L, 1, cb, a.U, p_old, a.r, be);
+            // all six loads before the first store: one L2 round trip instead of three (a load issued after a
+            // store that may alias it waits for that store)
+            C vp[3], vr[3];
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+                vp[c] = ld_coherent(p_old + (size_t)c * sVh + cb);
+                vr[c] = ld_coherent(a.r + (size_t)c * sVh + cb);
+            }
 #pragma unroll
             for (int c = 0; c < 3; ++c) {
                 a.t[(size_t)c * sVh + cb] = acc[c];
-                C vp = ld_coherent(p_old + (size_t)c * sVh + cb);
-                const C vr = ld_coherent(a.r + (size_t)c * sVh + cb);
-                vp.x = fma(be, vp.x, vr.x); vp.y = fma(be, vp.y, vr.y);
-                p_cur[(size_t)c * sVh + cb] = vp;
+                vp[c].x = fma(be, vp[c].x, vr[c].x); vp[c].y = fma(be, vp[c].y, vr[c].y);
+                p_cur[(size_t)c * sVh + cb] = vp[c];
             }
         }
         grid.sync();
@@ -145,14 +151,16 @@ __global__ void __launch_bounds__(PERSIST_BLOCK, 3) cg_persistent_kernel(const P
         for (int cb = gtid; cb < Vh; cb += gthreads) {
             C acc[3];
             persistent_site<T, NROW, TG, false>(acc, a.L, 0, cb, a.U, a.t);
+            C vv[3];
+#pragma unroll
+            for (int c = 0; c < 3; ++c) vv[c] = ld_coherent(p_cur + (size_t)c * sVh + cb);
 #pragma unroll
             for (int c = 0; c < 3; ++c) {
-                const C vv = ld_coherent(p_cur + (size_t)c * sVh + cb);
                 C o;
-                o.x = fma(a.m2, vv.x, -acc[c].x);
-                o.y = fma(a.m2, vv.y, -acc[c].y);
+                o.x = fma(a.m2, vv[c].x, -acc[c].x);
+                o.y = fma(a.m2, vv[c].y, -acc[c].y);
                 a.Ap[(size_t)c * sVh + cb] = o;
-                dot += (double)vv.x * (double)o.x + (double)vv.y * (double)o.y;
+                dot += (double)vv[c].x * (double)o.x + (double)vv[c].y * (double)o.y;
             }
         }
         {
