@@ -105,7 +105,10 @@ static cudaError_t launch_nrhs(const DslashLaunch &d)
     // staged kernel serves the (precision, NRHS, link rows) where it measured faster at 64^4
     // (profiles/README.md "staged vs register kernel"): fp64 n = 3, 4; fp32 n = 8, and n >= 4 on two-row links
     if constexpr (MODE != 1) {
-        constexpr bool staged_wins = sizeof(T) == 8 ? (NRHS == 3 || NRHS == 4) : (NRHS == 8 || (NROW == 2 && NRHS >= 4));
+        // (the reducing kernel, MODE 2, on full links is 3-5 % faster as the register kernel at n = 3, 4: 2.35 / 2.71 ms
+        // against 2.42 / 2.86 -- ncu shows the staged MODE 2 kernel requesting every link sector from the L2 twice)
+        constexpr bool staged_wins = sizeof(T) == 8 ? ((NRHS == 3 || NRHS == 4) && !(MODE == 2 && NROW == 3))
+                                                    : (NRHS == 8 || (NROW == 2 && NRHS >= 4));
         if (d.variant == 4 || (d.variant != 5 && staged_wins)) return launch_staged<T, MODE, NROW, TG, NRHS>(d);
     }
     if constexpr (NRHS == 1 && TG == 0) {
