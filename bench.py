@@ -1,7 +1,11 @@
 #!/usr/bin/env python
-"""bench.py -- staggered Dslash + CG hot path on B200 (one JSON line on stdout; rank 0 only).
+"""bench.py -- staggered Dslash + CG hot path on B200.
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--lattice 64,64,64,64] [--quick]
+
+stdout carries exactly ONE line: a compact (< 2 KB) JSON headline, printed last by rank 0.  Everything
+else the run measures (per-config table, full solves, variants, sweeps) goes to a sidecar JSON file whose
+path is in the headline (`extras`, default gpurun_out/bench_extras.json); progress goes to stderr.
 
 Workload (config.workload): BASELINE.json configs[4] -- 64^4 lattice, Haar-random SU(3) links
 (seed 0), Gaussian even-site source (seed 1), m = 0.01, fp64 -- the configuration the metric is
@@ -18,19 +22,23 @@ the stop test, the p update -- all in our CUDA kernels, scalars resident on the 
   e2e   : the same K iterations through the C-ABI with HOST buffers: qcd_field_upload of the
           source from pinned memory, K x (qcd_cg_iterate(1) + qcd_cg_poll, a 72-byte D2H read
           of the residual after every step), qcd_field_download of the iterate to pinned memory.
+          The gauge links are the operator, resident like model weights: their upload is outside.
   roofline : the Dslash kernel (D_oe launches inside the timed region, CUDA events on the
           launching stream), algorithmic = COMPULSORY DRAM bytes 1248 B/site (each link once,
           each spinor once, one store), against MEASURED_PEAKS.json hbm_gbs.
   cpu_baseline / --impl reference : the CPU oracle as it stands on the host cores.
 
 N > 1: replicas only: every rank runs the same workload on its own
-GPU, no data-path collective; value = sum of units / max-over-ranks device time.
+GPU, no data-path collective; value = sum of units / max-over-ranks device time.  `--gpus N`
+without a torchrun environment re-launches itself under torch.distributed.run with N ranks.
 """
 from __future__ import annotations
 
 import argparse
 import json
 import os
+import socket
+import subprocess
 import sys
 import threading
 import time
@@ -48,29 +56,53 @@ REALS_DSLASH_COMPULSORY = 156            # 8 links x 18 + 1 vector read + 1 writ
 REALS_ITER_NOMINAL = 2 * 198 + 6 + 36 + 18      # + epilogue read of p, x/r update (6 vectors), p update (3 vectors) = 456
 REALS_ITER_COMPULSORY = 2 * 156 + 6 + 36 + 18   # = 372 (2976 B fp64)
 THEORETICAL_HBM_GBS = 8184.0             # 3996 MHz x 2 (DDR) x 8192 bit / 8 -- nvidia-smi max memory clock; context only
+FLOP_PER_CG_ITER = 2 * FLOP_PER_SITE + 72     # per even site: two half-Dslash + m^2 p - (6 fma) + two dots (2 x 12) + x, r, p updates (3 x 12)
 
-METRIC = "staggered CG-iteration effective GB/s (two half-Dslash at 1584 B/site + CG vector kernels), 64^4 fp64"
 UNIT = "GB/s"
+HEADLINE_MAX_BYTES = 2000                # the driver keeps a tail of stdout: the line must survive it whole
+DEFAULT_EXTRAS = os.path.join("gpurun_out", "bench_extras.json")
 
 
-def parse_args():
+def lattice_name(dims) -> str:
+    d = tuple(dims)
+    return f"{d[0]}^4" if len(set(d)) == 1 else "x".join(map(str, d))
+
+
+def metric_name(dims, prec: int = 64) -> str:
+    return (f"staggered CG-iteration effective GB/s (two half-Dslash at {198 * prec // 8} B/site + CG vector kernels), "
+            f"{lattice_name(dims)} fp{prec}")
+
+
+def workload_name(dims, m, prec: int = 64) -> str:
+    return f"{'x'.join(map(str, dims))} staggered CG iteration, Haar links, m={m}, fp{prec}, full 18-real links"
+
+
+def log(msg: str) -> None:
+    print(f"[bench {time.strftime('%H:%M:%S')}] {msg}", file=sys.stderr, flush=True)
+
+
+def parse_args(argv=None):
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=200)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=("ours", "reference"))
     ap.add_argument("--lattice", default=None, help="override dims, e.g. 16,16,16,16 (testing only)")
-    ap.add_argument("--quick", action="store_true", help="skip the extra reports (full solves, fp32, cpu_baseline)")
+    ap.add_argument("--quick", action="store_true", help="headline only: no sidecar reports, no full solves, no cpu_baseline")
+    ap.add_argument("--extras", default=None, help=f"path of the sidecar JSON (default {DEFAULT_EXTRAS})")
     ap.add_argument("--variants-only", action="store_true",
                     help="run only the Dslash variant sweep (two-row / temporal gauge / NMULTI) and print it; used for ncu captures")
+    ap.add_argument("--dslash-only", action="store_true",
+                    help="run only `--reps` D_oe and D_eo launches of BASELINE.json configs[--config] in --prec; used for ncu captures")
+    ap.add_argument("--config", type=int, default=4, choices=(0, 1, 2, 3, 4), help="BASELINE.json config of --dslash-only")
     ap.add_argument("--prec", type=int, default=64, choices=(64, 32),
-                    help="precision of --variants-only, and of the timed CG iterations (32: the fp32 path of the same "
-                         "workload, reported with dtype f32 and without the extra reports; the default line is fp64)")
+                    help="precision of --variants-only / --dslash-only, and of the timed CG iterations (32: the fp32 path of "
+                         "the same workload, reported with dtype f32 and without the extra reports; the default line is fp64)")
     ap.add_argument("--nmulti", default="1,2,3,4,6,8", help="NMULTI values of --variants-only")
-    ap.add_argument("--reps", type=int, default=10, help="timed launches per variant of --variants-only")
+    ap.add_argument("--reps", type=int, default=10, help="timed launches per variant of --variants-only / --dslash-only")
     ap.add_argument("--kernel", type=int, default=0,
                     help="qcd_set_dslash_variant for --variants-only (0 default choice, 4 staged kernel, 5 register kernel)")
-    return ap.parse_args()
+    return ap.parse_args(argv)
 
 
 def load_peaks():
@@ -78,19 +110,21 @@ def load_peaks():
     if os.path.exists(p):
         with open(p) as f:
             d = json.load(f)
-        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, torch copy)"
+        return float(d["hbm_gbs"]), "MEASURED_PEAKS.json hbm_gbs (torch copy)"
     return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
 def load_traffic(prec: int):
-    """ncu-measured DRAM bytes per Dslash launch, recorded in profiles/ (text, committed); None if absent."""
+    """ncu-measured DRAM bytes of one D_oe launch at 64^4 and where they come from: profiles/dslash_traffic.csv
+    (text, committed; a constant from the capture named there, NOT a measurement of this run).  (None, None) if absent."""
     p = os.path.join(ROOT, "profiles", "dslash_traffic.csv")
     if not os.path.exists(p):
-        return None
+        return None, None
     with open(p) as f:
-        rows = dict(line.strip().split(",", 1) for line in f if "," in line)
+        rows = dict(line.strip().split(",", 1) for line in f if "," in line and not line.startswith("#"))
     v = rows.get(f"fp{prec}_64x64x64x64_bytes_per_launch")
-    return int(v) if v is not None else None
+    src = "profiles/dslash_traffic.csv (ncu --set full capture" + (f" at {rows['captured_at_commit']}" if "captured_at_commit" in rows else "") + ")"
+    return (int(v), src) if v is not None else (None, None)
 
 
 # ---- clocks ---------------------------------------------------------------------------------
@@ -158,6 +192,24 @@ def dist_env():
     return int(os.environ.get("RANK", 0)), int(os.environ.get("LOCAL_RANK", 0)), int(os.environ.get("WORLD_SIZE", 1))
 
 
+def free_port() -> int:
+    with socket.socket(socket.AF_INET, socket.SOCK_STREAM) as s:
+        s.bind(("127.0.0.1", 0))
+        return s.getsockname()[1]
+
+
+def respawn_under_torchrun(args, argv) -> int | None:
+    """`python bench.py --gpus N` with N > 1 and no torchrun environment: launch N ranks (one per GPU) of this very
+    command under torch.distributed.run and return its exit code; None when no re-launch is needed."""
+    if args.gpus <= 1 or "WORLD_SIZE" in os.environ or args.variants_only or args.dslash_only:
+        return None
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(args.gpus),
+           "--master-addr", "127.0.0.1", "--master-port", str(free_port()), os.path.abspath(__file__)] + list(argv)
+    env = dict(os.environ, MASTER_ADDR="127.0.0.1")
+    log(f"--gpus {args.gpus} without a torchrun environment: launching {args.gpus} ranks")
+    return subprocess.call(cmd, env=env, cwd=ROOT)
+
+
 def aggregate_over_ranks(local_ms: float, local_units: float, backend_device=None):
     """(max-over-ranks time, sum-over-ranks units).  No data-path collective exists; this is the
     only communication in the bench.  Works with gloo (CPU tensors) and nccl (CUDA tensors)."""
@@ -173,6 +225,44 @@ def aggregate_over_ranks(local_ms: float, local_units: float, backend_device=Non
     return float(t.item()), float(u.item())
 
 
+# ---- the one stdout line ---------------------------------------------------------------------
+HEADLINE_KEYS = ("impl", "metric", "value", "unit", "n_gpus", "steps", "warmup", "ms_per_step", "higher_is_better", "scaling",
+                 "vs_baseline", "dtype", "data", "config", "clocks", "e2e", "gpu_launches", "roofline", "cpu_baseline",
+                 "dslash_gbs_fp64", "dslash_frac_hbm_fp64", "dslash_gbs_fp32", "cg_s_per_solve_fp64", "cg_s_per_solve_fp32",
+                 "cg_iters_fp64", "extras")
+# dropped, in this order, if a line ever exceeds HEADLINE_MAX_BYTES (never the contract keys)
+HEADLINE_OPTIONAL = ("cg_iters_fp64", "data", "dslash_frac_hbm_fp64", "cg_s_per_solve_fp32", "dslash_gbs_fp32")
+
+
+def headline_line(out: dict) -> str:
+    """The compact JSON line: the bench contract's keys, the four numbers BASELINE.json's metric names and the
+    path of the sidecar.  Anything else in `out` stays in the sidecar."""
+    d = {k: out[k] for k in HEADLINE_KEYS if k in out}
+    line = json.dumps(d, separators=(",", ":"))
+    for k in HEADLINE_OPTIONAL:
+        if len(line) <= HEADLINE_MAX_BYTES:
+            break
+        d.pop(k, None)
+        line = json.dumps(d, separators=(",", ":"))
+    if len(line) > HEADLINE_MAX_BYTES:
+        raise RuntimeError(f"headline JSON is {len(line)} bytes (> {HEADLINE_MAX_BYTES}): trim a contract key's text")
+    return line
+
+
+def write_sidecar(path: str, data: dict) -> str | None:
+    try:
+        full = path if os.path.isabs(path) else os.path.join(ROOT, path)
+        os.makedirs(os.path.dirname(full), exist_ok=True)
+        tmp = full + f".tmp{os.getpid()}"
+        with open(tmp, "w") as f:
+            json.dump(data, f, indent=1)
+        os.replace(tmp, full)
+        return path
+    except OSError as e:  # a read-only checkout must not cost the headline
+        log(f"sidecar not written: {e!r}")
+        return None
+
+
 # ---- our arm ---------------------------------------------------------------------------------
 def make_inputs(dims, cfg_index=4):
     import qcd_inputs
@@ -181,244 +271,6 @@ def make_inputs(dims, cfg_index=4):
     U = qcd_inputs.gauge_field(cfg["dims"], cfg["links"], seed=0, eps=cfg["eps"])
     b = qcd_inputs.gaussian_source(cfg["dims"], seed=1, parity=0)
     return cfg, U, b
-
-
-def time_dslash(q, torch, ctx, fU, fin, fout, n=20):
-    for _ in range(3):
-        ctx.qcd_dslash_oe(fU, fout, fin)
-    torch.cuda.synchronize()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    e0.record()
-    for _ in range(n):
-        ctx.qcd_dslash_oe(fU, fout, fin)
-    e1.record()
-    torch.cuda.synchronize()
-    return e0.elapsed_time(e1) / n
-
-
-def variant_reals(nrow, tg, n, N3):
-    """(compulsory, nominal) reals per output site of one multi-vector half-Dslash:
-    links 6 * nrow reals each, 8 per site, or 6 + 2/N3 in temporal gauge (the time links are read only
-    on the slices x3 = 0 / 1); compulsory = each input vector once + each output once; nominal = all 8
-    neighbours of every vector (the paper's count: n 570 / (8 (6 12 + n 9 6)))."""
-    links = (6.0 + 2.0 / N3 if tg else 8.0) * 6 * nrow
-    return links + 12.0 * n, links + 54.0 * n
-
-
-def time_dslash_multi(torch, ctx, fU, fins, fouts, reps=10):
-    for _ in range(2 if reps > 1 else 0):
-        ctx.qcd_dslash_oe_multi(fU, fouts, fins)
-    torch.cuda.synchronize()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    e0.record()
-    for _ in range(reps):
-        ctx.qcd_dslash_oe_multi(fU, fouts, fins)
-    e1.record()
-    torch.cuda.synchronize()
-    return e0.elapsed_time(e1) / reps
-
-
-def variants_sweep(q, torch, ctx, fU_full, dims, peak, nmulti=(1, 2, 3, 4, 6, 8), reps=10):
-    """Dslash with the paper's traffic reductions, reported separately from the headline:
-    link storage x temporal gauge x NMULTI.  Throughput does not depend on the link values, so the
-    temporal-gauge rows run on the same links with the field marked (the kernel then skips the time links
-    of x3 != 0); correctness of every variant is tests/test_gpu_variants.py's job."""
-    Vh = int(np.prod(dims)) // 2
-    rsize = 8 if ctx.precision == 64 else 4
-    f12 = ctx.field(q.QCD_GAUGE_2ROW)
-    ctx.qcd_gauge_compress(fU_full, f12)
-    nmax = max(nmulti)
-    fins = [ctx.field(q.QCD_SPINOR_EVEN) for _ in range(nmax)]
-    fouts = [ctx.field(q.QCD_SPINOR_ODD) for _ in range(nmax)]
-    g = torch.Generator(device=ctx.device).manual_seed(7)
-    for f in fins:
-        real = torch.float64 if ctx.precision == 64 else torch.float32
-        f.buf.view(real).copy_(torch.randn(f.buf.numel() // rsize, generator=g, device=ctx.device, dtype=real))
-    rows = []
-    for name, fU, nrow, tg in (("full18", fU_full, 3, 0), ("tworow12", f12, 2, 0), ("tworow12+temporal_gauge", f12, 2, 1)):
-        ctx.qcd_gauge_set_temporal_unit(fU, bool(tg))
-        for n in nmulti:
-            ms = time_dslash_multi(torch, ctx, fU, fins[:n], fouts[:n], reps)
-            comp, nom = variant_reals(nrow, tg, n, dims[3])
-            gbs = comp * rsize * Vh / ms / 1e6
-            rows.append({"links": name, "nmulti": n, "ms": round(ms, 5),
-                         "tflops": round(FLOP_PER_SITE * n * Vh / ms / 1e9, 3),
-                         "gbs_compulsory": round(gbs, 1), "frac_of_measured_copy_peak": round(gbs / peak, 4),
-                         "ai_nominal_flop_per_byte": round(FLOP_PER_SITE * n / (nom * rsize), 3),
-                         # Eq. (2) of the paper (PAPER.md:70-74): attainable = min(peak, AI x bandwidth); the
-                         # bandwidth term binds at every n here.  With the paper's NOMINAL bytes (no cache reuse
-                         # of the neighbour vectors) a kernel whose L2 serves that reuse lands ABOVE this line,
-                         # as the paper observes on A100 (PAPER.md:100); with compulsory bytes it cannot.
-                         "eq2_attainable_tflops_nominal_ai": round(FLOP_PER_SITE * n / (nom * rsize) * peak / 1e3, 3),
-                         "eq2_attainable_tflops_compulsory_ai": round(FLOP_PER_SITE * n / (comp * rsize) * peak / 1e3, 3)})
-        ctx.qcd_gauge_set_temporal_unit(fU, False)
-    for f in fins + fouts + [f12]:
-        f.free()
-    return rows
-
-
-def cg_multi_report(q, torch, device, dims, prec, fU_full, m, ns=(1, 2, 4), iters=20):
-    """n CG solves in lock step (qcd_cg_begin_multi / qcd_cg_iterate): ms per iteration and per right-hand side,
-    on the paper's link storage (two rows + temporal gauge marking) and on full links."""
-    rows = []
-    ctx0 = fU_full.ctx
-    for n in ns:
-        ctx = q.Context(dims, prec, device=device, nrhs=n)
-        fb = [ctx.field(q.QCD_SPINOR_EVEN) for _ in range(n)]
-        fx = [ctx.field(q.QCD_SPINOR_EVEN) for _ in range(n)]
-        real = torch.float64 if prec == 64 else torch.float32
-        g = torch.Generator(device=device).manual_seed(11)
-        for f in fb:
-            f.buf.view(real).copy_(torch.randn(f.buf.numel() // (prec // 8), generator=g, device=device, dtype=real))
-        for name, kind in (("full18", q.QCD_GAUGE), ("tworow12+temporal_gauge", q.QCD_GAUGE_2ROW)):
-            if kind == q.QCD_GAUGE:
-                fU = ctx.field(kind, buf=fU_full.buf)      # same device memory, descriptor of the new context
-            else:
-                f12 = ctx0.field(q.QCD_GAUGE_2ROW)
-                ctx0.qcd_gauge_compress(fU_full, f12)
-                fU = ctx.field(kind, buf=f12.buf)
-            ctx.qcd_gauge_set_temporal_unit(fU, kind == q.QCD_GAUGE_2ROW)
-            ctx.qcd_cg_begin_multi(fU, fb, fx, m, 1e-300, 1 << 30)
-            ctx.qcd_cg_iterate(3)
-            torch.cuda.synchronize()
-            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            e0.record()
-            ctx.qcd_cg_iterate(iters)
-            e1.record()
-            torch.cuda.synchronize()
-            ctx.qcd_cg_finish_multi()
-            ms = e0.elapsed_time(e1) / iters
-            rows.append({"links": name, "n": n, "ms_per_iter": round(ms, 5), "ms_per_iter_per_rhs": round(ms / n, 5)})
-            fU.free()
-        for f in fb + fx:
-            f.free()
-        ctx.close()
-        torch.cuda.empty_cache()
-    return rows
-
-
-def small_lattice_report(q, torch, device):
-    """configs[1] (16^4, links fit the L2): the solve is launch- and reduction-latency bound.
-    The three solver loops of qcd_set_cg_loop: kernel-by-kernel enqueue, CUDA-graph replay of 16 iterations
-    (side stream), and the persistent cooperative kernel (the library's choice at this size)."""
-    dims = (16, 16, 16, 16)
-    cfg, U, b = make_inputs(dims, 1)
-    rows = []
-    stream = torch.cuda.Stream(device=device)
-    with torch.cuda.stream(stream):
-        for prec, tol in ((64, cfg["tol64"]), (32, cfg["tol32"])):
-            ctx = q.Context(dims, prec, stream=stream, device=device)
-            fU = ctx.field(q.QCD_GAUGE).upload(U)
-            fb = ctx.field(q.QCD_SPINOR_EVEN).upload(b)
-            fx = ctx.field(q.QCD_SPINOR_EVEN)
-            for loop, name in ((1, "kernel-by-kernel enqueue"), (2, "CUDA-graph replay, 16 iterations per launch"),
-                               (3, "persistent cooperative kernel (one launch per solve)")):
-                ctx.qcd_set_cg_loop(loop)
-                ctx.qcd_cg_solve(fU, fb, fx, cfg["m"], tol, cfg["maxiter"])
-                best = None
-                for _ in range(3):
-                    t0 = time.perf_counter()
-                    info = ctx.qcd_cg_solve(fU, fb, fx, cfg["m"], tol, cfg["maxiter"])
-                    wall = time.perf_counter() - t0
-                    if best is None or info["seconds"] < best[0]["seconds"]:
-                        best = (info, wall)
-                info, wall = best
-                rows.append({"loop": name, "prec": prec, "tol": tol, "iters": info["iters"], "converged": info["converged"],
-                             "ms_per_solve_device": round(1e3 * info["seconds"], 4), "ms_per_solve_wall": round(1e3 * wall, 4),
-                             "us_per_iter": round(1e6 * info["seconds"] / max(info["iters"], 1), 3)})
-            ctx.close()
-    return {"lattice": list(dims), "rows": rows}
-
-
-FLOP_PER_CG_ITER = 2 * FLOP_PER_SITE + 72     # per even site: two half-Dslash + m^2 p - (6 fma) + two dots (2 x 12) + x, r, p updates (3 x 12)
-
-
-def size_sweep_report(q, torch, device, sizes=((8, 8, 8, 8), (12, 12, 12, 12), (16, 16, 16, 16), (24, 24, 24, 24),
-                                               (32, 32, 32, 32), (48, 48, 48, 12), (32, 32, 64, 64)), iters=200):
-    """The paper's Fig. 3 experiment: Dslash and CG throughput against the lattice size, in
-    single and double precision (the 64^4 point is the headline above; 32^2 x 64^2 is the size beyond which the
-    paper's MI250X curve degrades, PAPER.md:54).  Dslash: 20 back-to-back D_oe launches;
-    CG: qcd_cg_solve with an unreachable tolerance and maxiter = `iters`, i.e. the solver loop the library picks
-    for that size (persistent kernel while the lattice fits the L2, kernel-by-kernel beyond).  GFLOP/s with
-    570 flop per site (Dslash) and 2 x 570 + 72 flop per even site and iteration (CG)."""
-    import qcd_inputs
-    rows = []
-    for dims in sizes:
-        Vh = int(np.prod(dims)) // 2
-        U = qcd_inputs.gauge_field(dims, "haar", seed=0)
-        b = qcd_inputs.gaussian_source(dims, seed=1)
-        for prec in (64, 32):
-            stream = torch.cuda.Stream(device=device)
-            with torch.cuda.stream(stream):
-                ctx = q.Context(dims, prec, device=device, stream=stream)
-                fU = ctx.field(q.QCD_GAUGE).upload(U)
-                fb = ctx.field(q.QCD_SPINOR_EVEN).upload(b)
-                fx = ctx.field(q.QCD_SPINOR_EVEN)
-                fo = ctx.field(q.QCD_SPINOR_ODD)
-                # 20 launches captured in one CUDA graph: below 16^4 a Python-driven launch loop would
-                # time the host, not the kernel
-                ctx.qcd_dslash_oe(fU, fo, fb)
-                stream.synchronize()
-                graph = torch.cuda.CUDAGraph()
-                with torch.cuda.graph(graph, stream=stream):
-                    for _ in range(20):
-                        ctx.qcd_dslash_oe(fU, fo, fb)
-                graph.replay()
-                stream.synchronize()
-                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-                e0.record(stream)
-                for _ in range(5):
-                    graph.replay()
-                e1.record(stream)
-                stream.synchronize()
-                ms_d = e0.elapsed_time(e1) / 100
-                del graph
-            ctx.qcd_cg_solve(fU, fb, fx, 0.01, 1e-300, 20)
-            secs = min(ctx.qcd_cg_solve(fU, fb, fx, 0.01, 1e-300, iters)["seconds"] for _ in range(2))
-            rows.append({"lattice": list(dims), "prec": prec, "dslash_us": round(1e3 * ms_d, 3),
-                         "dslash_gflops": round(FLOP_PER_SITE * Vh / ms_d / 1e6, 1),
-                         "cg_us_per_iter": round(1e6 * secs / iters, 3),
-                         "cg_gflops": round(FLOP_PER_CG_ITER * Vh * iters / secs / 1e9, 1)})
-            ctx.close()
-    return rows
-
-
-def update_routine_report(q, torch, device, peak, dims=(48, 48, 48, 48), iters=50):
-    """The paper's Table 1 workload: bandwidth of the "CG update routine" on a 48^4 lattice,
-    fp64 -- here the fused x += alpha p, r -= alpha Ap, |r|^2 kernel (288 B per even site) and the p update
-    (144 B), timed by CUDA events around each launch inside running CG iterations."""
-    cfg, U, b = make_inputs(dims, 4)
-    Vh = int(np.prod(dims)) // 2
-    ctx = q.Context(dims, 64, device=device)
-    fU = ctx.field(q.QCD_GAUGE).upload(U)
-    fb = ctx.field(q.QCD_SPINOR_EVEN).upload(b)
-    fx = ctx.field(q.QCD_SPINOR_EVEN)
-    ctx.qcd_cg_begin(fU, fb, fx, cfg["m"], 1e-300, 1 << 30)
-    ctx.qcd_cg_iterate(5)
-    ctx.qcd_profile_enable(True)
-    ctx.qcd_cg_iterate(iters)
-    n_xr, ms_xr = ctx.qcd_profile_read(q.QCD_K_UPDATE_XR)
-    n_p, ms_p = ctx.qcd_profile_read(q.QCD_K_UPDATE_P)
-    ctx.qcd_profile_enable(False)
-    ctx.qcd_cg_finish()
-    ctx.close()
-    xr = 36 * 8 * Vh / (ms_xr / n_xr) / 1e6
-    pu = 18 * 8 * Vh / (ms_p / n_p) / 1e6
-    return {"lattice": list(dims), "update_xr_norm_ms": round(ms_xr / n_xr, 5), "update_xr_norm_gbs": round(xr, 1),
-            "update_xr_frac_of_measured_copy_peak": round(xr / peak, 4), "update_p_ms": round(ms_p / n_p, 5),
-            "update_p_gbs": round(pu, 1),
-            "paper_table1_gbs": {"OpenCL on A100": 1351, "CUDA on A100": 1317, "OpenCL on MI250x": 1134,
-                                 "peaks": {"A100": 1555, "MI250x GCD": 1638},
-                                 "source": "PAPER.md:56-62 (other hardware; context only)"}}
-
-
-def dslash_report(ms, Vh, rsize, peak):
-    comp = REALS_DSLASH_COMPULSORY * rsize * Vh / ms / 1e6
-    return {"ms": round(ms, 5), "gflops": round(FLOP_PER_SITE * Vh / ms / 1e6, 1),
-            "effective_gbs_nominal": round(REALS_DSLASH_NOMINAL * rsize * Vh / ms / 1e6, 1),
-            "gbs_compulsory": round(comp, 1),
-            "frac_of_measured_copy_peak": round(comp / peak, 4),
-            "frac_of_theoretical_8184": round(comp / THEORETICAL_HBM_GBS, 4)}
 
 
 def run_ours(args):
@@ -448,6 +300,7 @@ def run_ours(args):
     fx = ctx.field(q.QCD_SPINOR_EVEN)
     fo = ctx.field(q.QCD_SPINOR_ODD)
     if rank == 0:
+        log(f"generating {lattice_name(dims)} inputs")
         cfg, U, b = make_inputs(dims)
         fU.upload(U)
         fb.upload(b)
@@ -464,7 +317,7 @@ def run_ours(args):
         dist.broadcast(fb.buf, src=0)
         if rank != 0:
             b = fb.download()                  # the canonical host source (for the e2e leg) through the library
-    m, tol64 = cfg["m"], cfg["tol64"]
+    m = cfg["m"]
     t_setup = time.time() - t_setup
 
     def barrier():
@@ -473,6 +326,7 @@ def run_ours(args):
             dist.barrier()
 
     # ---------------- timed region: K CG iterations, inputs resident --------------------------
+    log(f"timed region: {W} + {K} CG iterations")
     ctx.qcd_cg_begin(fU, fb, fx, m, 1e-300, 1 << 30)      # tol far below reach: every step does full work
     ctx.qcd_cg_iterate(W)
     barrier()
@@ -507,10 +361,9 @@ def run_ours(args):
     e0.record()
     ctx._check(ctx.lib.qcd_field_upload(fb.handle, hb.data_ptr()), "qcd_field_upload")
     ctx.qcd_cg_begin(fU, fb, fx, m, 1e-300, 1 << 30)
-    rr_last = None
     for _ in range(K):
         ctx.qcd_cg_iterate(1)
-        _, _, rr_last = ctx.qcd_cg_poll()                  # D2H read of the step's result (residual)
+        ctx.qcd_cg_poll()                                  # D2H read of the step's result (residual)
     ctx.qcd_cg_finish()
     ctx._check(ctx.lib.qcd_field_download(fx.handle, hx.data_ptr()), "qcd_field_download")
     e1.record()
@@ -522,9 +375,8 @@ def run_ours(args):
     e2e = {"value": round(e2e_units / e2e_ms_max / 1e6, 2), "unit": UNIT,
            "h2d_bytes_per_step": int(spinor_host_bytes / K), "d2h_bytes_per_step": int(spinor_host_bytes / K + 72),
            "ms_total": round(e2e_ms_max, 3),
-           "what": "qcd_field_upload(b, pinned host) + K x [qcd_cg_iterate(1) + qcd_cg_poll (D2H of the residual)] + "
-                   "qcd_field_download(x, pinned host); host copies amortised over the K steps of the solve"}
-    del hb, hx
+           "what": "upload(b, pinned) + K x [qcd_cg_iterate(1) + qcd_cg_poll D2H] + download(x); source/solution copies "
+                   "amortised over K; the 9.7 GB link upload (the operator, resident) is outside"}
 
     # ---------------- roofline of the dominant kernel ------------------------------------------
     n_ds, ms_ds = prof[q.QCD_K_DSLASH]
@@ -535,9 +387,10 @@ def run_ours(args):
     # copy peak and the theoretical peak
     ctx.qcd_stream_read(fU, 3)
     stream_gbs = fU.nbytes / ctx.qcd_stream_read(fU, 10) / 1e6
+    traffic, traffic_src = load_traffic(prec) if dims == (64, 64, 64, 64) else (None, None)
     roofline = {"bound": "hbm", "kernel": f"dslash_kernel<{'double' if prec == 64 else 'float'},MODE0> (D_oe inside the CG iteration)",
                 "achieved": round(achieved, 1), "peak": peak, "unit": "GB/s", "frac": round(achieved / peak, 4),
-                "peak_source": peak_src, "traffic": load_traffic(prec) if dims == (64, 64, 64, 64) else None,
+                "peak_source": peak_src, "traffic": traffic, "traffic_source": traffic_src,
                 "algorithmic_bytes_per_launch": REALS_DSLASH_COMPULSORY * rsize * Vh,
                 "avg_launch_ms": round(ds_ms, 5), "launches_timed": n_ds,
                 "frac_of_theoretical_8184": round(achieved / THEORETICAL_HBM_GBS, 4),
@@ -547,156 +400,49 @@ def run_ours(args):
                   ("update_xr_norm", q.QCD_K_UPDATE_XR), ("update_p", q.QCD_K_UPDATE_P))}
 
     out = {
-        "metric": METRIC if prec == 64 else METRIC.replace("fp64", "fp32").replace("1584", "792"),
+        "metric": metric_name(dims, prec),
         "value": round(value, 2), "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
         "ms_per_step": round(ms_max / K, 5), "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-        "dtype": f"f{prec}", "data": "synthetic (seeded Haar SU(3) links, Gaussian source; BASELINE.json configs[4])",
-        "config": {"workload": f"{'x'.join(map(str, dims))} staggered CG iteration, Haar links, m={m}, fp{prec}, full 18-real links",
-                   "lattice": list(dims), "sites": V, "l2": "inputs (9.7 GB links) >> 126 MB L2, no flush needed",
-                   "parallelism": "replicas only (no data-path collective)" if world > 1 else "single GPU",
-                   "bytes_per_even_site_per_step": REALS_ITER_NOMINAL * rsize},
+        "dtype": f"f{prec}", "data": "synthetic: seeded Haar SU(3) links, Gaussian source (BASELINE.json configs[4])",
+        "config": {"workload": workload_name(dims, m, prec),
+                   "l2": "inputs (9.7 GB links) >> 126 MB L2, no flush needed" if V >= 1 << 22 else "small lattice: L2-resident",
+                   "parallelism": "replicas only (no data-path collective)" if world > 1 else "single GPU"},
         "clocks": clocks.summary(), "e2e": e2e, "gpu_launches": int(launches),
-        "roofline": roofline, "kernel_ms": kernel_ms, "setup_seconds": round(t_setup, 1),
+        "roofline": roofline,
     }
+    side = dict(out)
+    side.update({"kernel_ms": kernel_ms, "setup_seconds": round(t_setup, 1), "lattice": list(dims), "sites": V,
+                 "bytes_per_even_site_per_step": REALS_ITER_NOMINAL * rsize})
 
     if rank == 0 and not args.quick and prec == 64:
-        extras(args, q, torch, ctx, out, cfg, dims, U, b, fU, fb, fx, fo, peak)
+        import bench_reports
+        bench_reports.run_all(args, q, torch, ctx, out, side, cfg, dims, U, b, hb, hx, fU, fb, fx, fo, peak, stream_gbs)
+    del hb, hx
     if rank == 0:
-        print(json.dumps(out), flush=True)
-    ctx.close()
+        path = write_sidecar(args.extras or DEFAULT_EXTRAS, side)
+        if path:
+            out["extras"] = path
+        print(headline_line(out), flush=True)
+    try:
+        ctx.close()
+    except Exception:
+        pass
     if world > 1:
         import torch.distributed as dist
         dist.destroy_process_group()
 
 
-def extras(args, q, torch, ctx, out, cfg, dims, U, b, fU, fb, fx, fo, peak):
-    """Reports beside the headline (rank 0, N = 1 semantics): Dslash alone, full solves, fp32, oracle."""
-    import oracle
-    V = int(np.prod(dims))
-    Vh = V // 2
-    m = cfg["m"]
-    # Dslash alone, fp64
-    out["dslash_fp64"] = dslash_report(time_dslash(q, torch, ctx, fU, fb, fo), Vh, 8, peak)
-    # full fp64 solve: CG s/solve (BASELINE.json metric)
-    info = ctx.qcd_cg_solve(fU, fb, fx, m, cfg["tol64"], cfg["maxiter"])
-    x64 = fx.download()
-    t0 = time.time()
-    true64 = oracle.true_residual(dims, U, b, x64, m)
-    t_true = time.time() - t0
-    out["cg_fp64"] = {"tol": cfg["tol64"], "iters": info["iters"], "converged": info["converged"],
-                      "s_per_solve": round(info["seconds"], 4),
-                      "ms_per_iter": round(1e3 * info["seconds"] / max(info["iters"], 1), 5),
-                      "rel_resid_recurrence": info["rel_resid"], "true_resid_oracle_fp64": true64}
-    # CPU baseline: the oracle as it stands, a bounded sample of the same workload
-    nit = 12                                                # ~10 s of oracle time at 64^4 on 16 cores
-    t0 = time.time()
-    _, oinfo = oracle.cg(dims, U, b, m, 1e-300, nit)
-    t_or = time.time() - t0
-    out["cpu_baseline"] = {"value": round(REALS_ITER_NOMINAL * 8 * Vh * oinfo["iters"] / t_or / 1e9, 3), "unit": UNIT,
-                           "cores": oracle.num_threads(), "kind": "oracle",
-                           "sample": f"{nit} CG iterations (maxiter={nit}) of the same {'x'.join(map(str, dims))} fp64 solve, "
-                                     f"including the oracle's own set-up; {t_or:.1f} s",
-                           "oracle_apply_M_seconds": round(t_true, 2)}
-    del x64
-    # ---- variants, reported separately from the headline (SURVEY.md Sec. 8(f); PAPER.md:76-78) ----
-    c32 = q.Context(dims, 32, device=ctx.device)
-    gU = c32.field(q.QCD_GAUGE)
-    ctx.qcd_field_convert(gU, fU)                          # fp32 links = round-to-nearest of the fp64 links, on the device
-    gx = c32.field(q.QCD_SPINOR_EVEN)
-    go = c32.field(q.QCD_SPINOR_ODD)
-    # mixed-precision defect-correction CG to the fp64 tolerance (DESIGN.md R21)
-    inner_tol = 1e-3
-    mi = ctx.qcd_cg_solve_mixed(c32, fU, gU, fb, fx, gx, c32.field(q.QCD_SPINOR_EVEN), m, cfg["tol64"], inner_tol,
-                                4 * cfg["maxiter"])
-    xm = fx.download()
-    out["cg_mixed"] = {"tol": cfg["tol64"], "inner_tol": inner_tol, "converged": mi["converged"], "outer": mi["outer"],
-                       "inner_iters_fp32": mi["inner_iters"], "m_applications_fp64": mi["m_applications_fp64"],
-                       "s_per_solve": round(mi["seconds"], 4), "true_resid_device_fp64": mi["true_resid"],
-                       "true_resid_oracle_fp64": oracle.true_residual(dims, U, b, xm, m),
-                       "speedup_vs_cg_fp64": round(out["cg_fp64"]["s_per_solve"] / max(mi["seconds"], 1e-9), 3)}
-    del xm
-    # the same two solves on the paper's link storage (PAPER.md:76): temporal gauge fixed on the device,
-    # two rows stored; the source is rotated in (b' = g b), the solution rotated back (x = g^dagger x'),
-    # and the oracle checks the residual against the ORIGINAL links and source
-    fUf, fg = ctx.field(q.QCD_GAUGE), ctx.field(q.QCD_COLOUR_MATRIX)
-    ctx.qcd_gauge_fix_temporal(fU, fUf, fg)
-    f12 = ctx.field(q.QCD_GAUGE_2ROW)
-    ctx.qcd_gauge_compress(fUf, f12)
-    fUf.free()
-    g12 = c32.field(q.QCD_GAUGE_2ROW)
-    ctx.qcd_field_convert(g12, f12)
-    fbr = ctx.field(q.QCD_SPINOR_EVEN)
-    ctx.qcd_spinor_rotate(fg, fbr, fb)
-    info = ctx.qcd_cg_solve(f12, fbr, fx, m, cfg["tol64"], cfg["maxiter"])
-    ctx.qcd_spinor_rotate(fg, fx, fx, dagger=True)
-    xc = fx.download()
-    out["cg_fp64_tworow_temporal_gauge"] = {
-        "tol": cfg["tol64"], "iters": info["iters"], "converged": info["converged"], "s_per_solve": round(info["seconds"], 4),
-        "ms_per_iter": round(1e3 * info["seconds"] / max(info["iters"], 1), 5),
-        "true_resid_oracle_fp64_original_links": oracle.true_residual(dims, U, b, xc, m),
-        "speedup_vs_cg_fp64": round(out["cg_fp64"]["s_per_solve"] / max(info["seconds"], 1e-9), 3)}
-    mi = ctx.qcd_cg_solve_mixed(c32, f12, g12, fbr, fx, gx, c32.field(q.QCD_SPINOR_EVEN), m, cfg["tol64"], inner_tol,
-                                4 * cfg["maxiter"])
-    ctx.qcd_spinor_rotate(fg, fx, fx, dagger=True)
-    xc = fx.download()
-    out["cg_mixed_tworow_temporal_gauge"] = {
-        "tol": cfg["tol64"], "inner_tol": inner_tol, "converged": mi["converged"], "outer": mi["outer"],
-        "inner_iters_fp32": mi["inner_iters"], "s_per_solve": round(mi["seconds"], 4),
-        "true_resid_device_fp64": mi["true_resid"],
-        "true_resid_oracle_fp64_original_links": oracle.true_residual(dims, U, b, xc, m),
-        "speedup_vs_cg_fp64": round(out["cg_fp64"]["s_per_solve"] / max(mi["seconds"], 1e-9), 3)}
-    del xc
-    for f in (f12, g12, fg, fbr):
-        f.free()
-    out["variants_fp64"] = {"lattice": list(dims), "dslash": variants_sweep(q, torch, ctx, fU, dims, peak)}
-    out["cg_multi_fp64"] = cg_multi_report(q, torch, ctx.device, dims, 64, fU, m)
-    # fp32: free the fp64 device fields first
-    fU.free(); fb.free(); fx.free(); fo.free()
-    ctx.close()
-    torch.cuda.empty_cache()
-    U32, b32 = U.astype(np.complex64), b.astype(np.complex64)
-    gb = c32.field(q.QCD_SPINOR_EVEN).upload(b32)
-    out["dslash_fp32"] = dslash_report(time_dslash(q, torch, c32, gU, gb, go), Vh, 4, peak)
-    out["variants_fp32"] = {"lattice": list(dims), "dslash": variants_sweep(q, torch, c32, gU, dims, peak)}
-    if cfg["tol32"]:
-        info = c32.qcd_cg_solve(gU, gb, gx, m, cfg["tol32"], cfg["maxiter"])
-        x32 = gx.download()
-        out["cg_fp32"] = {"tol": cfg["tol32"], "iters": info["iters"], "converged": info["converged"],
-                          "s_per_solve": round(info["seconds"], 4),
-                          "ms_per_iter": round(1e3 * info["seconds"] / max(info["iters"], 1), 5),
-                          "rel_resid_recurrence": info["rel_resid"],
-                          "true_resid_oracle_fp64": oracle.true_residual(dims, U32, b32, x32, m),
-                          "note": "plain fp32 CG on Haar links stalls in TRUE residual near 1e-4 (DESIGN.md R11)"}
-    c32.close()
-    torch.cuda.empty_cache()
-    # the paper's own NMULTI experiment: 32^4, two-row links, temporal gauge (PAPER.md:76-98, Table 2)
-    if dims == (64, 64, 64, 64):
-        d32 = (32, 32, 32, 32)
-        _, U_32, _ = make_inputs(d32, 2)
-        t2 = {"lattice": list(d32), "paper_A100_tflops": {"fp32": {1: 2.244, 2: 2.532, 3: 2.953, 4: 3.205, 6: 3.090, 8: 3.006},
-                                                           "fp64": {1: 1.245, 2: 1.530, 3: 1.929, 4: 2.199, 6: 2.039, 8: 2.026},
-                                                           "source": "PAPER.md:84-98 Table 2 (A100, OpenCL; other hardware, context only)"}}
-        for prec in (64, 32):
-            c = q.Context(d32, prec, device=ctx.device)
-            f = c.field(q.QCD_GAUGE).upload(U_32)
-            t2[f"fp{prec}"] = variants_sweep(q, torch, c, f, d32, peak)
-            f.free(); c.close()
-        out["variants_table2_32x32x32x32"] = t2
-        out["cg_small_lattice"] = small_lattice_report(q, torch, ctx.device)
-        out["cg_update_routine_48x48x48x48"] = update_routine_report(q, torch, ctx.device, peak)
-        out["size_sweep_fig3"] = size_sweep_report(q, torch, ctx.device)
-    out["paper_context"] = {"A100_OpenCL_dslash_fp64_TFLOPs_32^4_12real_links_gaugefixed": 1.245,
-                            "A100_OpenCL_cg_update_GBs_48^4_fp64": 1351, "source": "PAPER.md:59,87 (other hardware; context only)"}
-
-
 # ---- reference arm: the CPU oracle -------------------------------------------------------------
 def run_reference(args):
+    """The oracle as it stands, on the host cores, on OUR arm's workload (64^4 unless --lattice says otherwise):
+    W untimed + K timed CG iterations of the same solve (a bounded sample of it: iterations, not sites)."""
     rank, _, world = dist_env()
     if rank != 0:
         return
     import oracle
     K, W = args.steps, args.warmup
-    dims = tuple(int(v) for v in args.lattice.split(",")) if args.lattice else (32, 32, 32, 32)
+    dims = tuple(int(v) for v in args.lattice.split(",")) if args.lattice else (64, 64, 64, 64)
+    log(f"reference arm: generating {lattice_name(dims)} inputs")
     cfg, U, b = make_inputs(dims)
     Vh = int(np.prod(dims)) // 2
     if W > 0:
@@ -705,22 +451,23 @@ def run_reference(args):
     _, info = oracle.cg(dims, U, b, cfg["m"], 1e-300, K)
     dt = time.perf_counter() - t0
     value = REALS_ITER_NOMINAL * 8 * Vh * info["iters"] / dt / 1e9
-    sample = (f"{K} CG iterations of the CPU oracle on a {'x'.join(map(str, dims))} lattice of the same recipe "
-              f"(Haar links, m={cfg['m']}, fp64): a 1/{(64 ** 4) // int(np.prod(dims))} sample of the 64^4 sites; GB/s is per-site intensive")
-    out = {"impl": "reference", "metric": METRIC, "value": round(value, 4), "unit": UNIT, "n_gpus": world, "steps": K,
+    sample = (f"{K} CG iterations (after {W} untimed) of the CPU oracle on the same {'x'.join(map(str, dims))} solve, "
+              f"oracle set-up included; {dt:.1f} s")
+    out = {"impl": "reference", "metric": metric_name(dims), "value": round(value, 4), "unit": UNIT,
+           "n_gpus": max(world, args.gpus), "steps": K,
            "warmup": W, "ms_per_step": round(1e3 * dt / max(info["iters"], 1), 3), "higher_is_better": True,
            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic (seeded)",
-           "config": {"workload": "64x64x64x64 staggered CG iteration, Haar links, m=0.01, fp64, full 18-real links",
-                      "sample": sample},
+           "config": {"workload": workload_name(dims, cfg["m"]), "sample": sample},
            "cpu_baseline": {"value": round(value, 4), "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle", "sample": sample},
            "e2e": {"value": round(value, 4), "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
            "gpu_launches": 0}
-    print(json.dumps(out), flush=True)
+    print(headline_line(out), flush=True)
 
 
 def run_variants_only(args):
     """Dslash variant sweep alone (rank 0, one GPU): `--lattice`, `--prec`, `--nmulti`, `--reps`."""
     import torch
+    import bench_reports
     import paper_2502_03249_b200 as q
     dims = tuple(int(v) for v in args.lattice.split(",")) if args.lattice else (64, 64, 64, 64)
     peak, _ = load_peaks()
@@ -728,15 +475,52 @@ def run_variants_only(args):
     ctx = q.Context(dims, args.prec)
     fU = ctx.field(q.QCD_GAUGE).upload(U)
     ctx.qcd_set_dslash_variant(args.kernel)
-    rows = variants_sweep(q, torch, ctx, fU, dims, peak, tuple(int(v) for v in args.nmulti.split(",")), args.reps)
+    rows = bench_reports.variants_sweep(q, torch, ctx, fU, dims, peak, tuple(int(v) for v in args.nmulti.split(",")), args.reps)
     print(json.dumps({"variants": rows, "lattice": list(dims), "prec": args.prec, "gpu_launches": ctx.qcd_launch_count()}), flush=True)
     ctx.close()
 
 
-def main():
-    args = parse_args()
+def run_dslash_only(args):
+    """`--reps` launches each of D_oe and D_eo (and one qcd_apply_M) at BASELINE.json configs[--config]: the command the
+    per-config ncu captures under profiles/ are taken with."""
+    import torch
+    import qcd_inputs
+    import paper_2502_03249_b200 as q
+    cfg, U, b = qcd_inputs.config_inputs(args.config)
+    if args.lattice:
+        cfg, U, b = qcd_inputs.config_inputs(args.config, tuple(int(v) for v in args.lattice.split(",")))
+    dims = cfg["dims"]
+    ctx = q.Context(dims, args.prec)
+    fU = ctx.field(q.QCD_GAUGE).upload(U)
+    fb = ctx.field(q.QCD_SPINOR_EVEN).upload(b)
+    fo, fe = ctx.field(q.QCD_SPINOR_ODD), ctx.field(q.QCD_SPINOR_EVEN)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ctx.qcd_dslash_oe(fU, fo, fb)
+    torch.cuda.synchronize()
+    e0.record()
+    for _ in range(args.reps):
+        ctx.qcd_dslash_oe(fU, fo, fb)
+        ctx.qcd_dslash_eo(fU, fe, fo)
+    e1.record()
+    torch.cuda.synchronize()
+    ctx.qcd_apply_M(fU, fe, fb, cfg["m"])
+    torch.cuda.synchronize()
+    print(json.dumps({"dslash_only": True, "config": args.config, "lattice": list(dims), "prec": args.prec,
+                      "ms_per_half_dslash": round(e0.elapsed_time(e1) / (2 * args.reps), 5),
+                      "gpu_launches": ctx.qcd_launch_count()}), flush=True)
+    ctx.close()
+
+
+def main(argv=None):
+    argv = sys.argv[1:] if argv is None else argv
+    args = parse_args(argv)
+    rc = respawn_under_torchrun(args, argv)
+    if rc is not None:
+        sys.exit(rc)
     if args.variants_only:
         run_variants_only(args)
+    elif args.dslash_only:
+        run_dslash_only(args)
     elif args.impl == "reference":
         run_reference(args)
     else:

@@ -145,7 +145,9 @@ qcd_status qcd_set_workspace(qcd_ctx *ctx, void *device_ptr, size_t nbytes);
  * Parity blocks of Eq. (1).  Asynchronous on the context stream.
  *   qcd_dslash_eo : out_even = D_eo in_odd      qcd_dslash_oe : out_odd = D_oe in_even
  * U is a QCD_GAUGE field.  out must not alias in.  Kind mismatch -> QCD_EINVAL.
- * A QCD_SPINOR_FULL field may be passed for either argument: its even or odd half is used.
+ * A QCD_SPINOR_FULL field may be passed for either argument: its even or odd half is used (the two halves of
+ * ONE full field are distinct memory, so the same full field may serve as out and in).  Aliasing is checked on
+ * byte ranges of the half-fields, not on base pointers.
  */
 qcd_status qcd_dslash_eo(qcd_ctx *ctx, const qcd_field *U, qcd_field *out_even, const qcd_field *in_odd);
 qcd_status qcd_dslash_oe(qcd_ctx *ctx, const qcd_field *U, qcd_field *out_odd, const qcd_field *in_even);
@@ -166,6 +168,9 @@ qcd_status qcd_apply_M(qcd_ctx *ctx, const qcd_field *U, qcd_field *out_even, co
  * Returns QCD_OK (converged), QCD_ENOTCONVERGED, QCD_EBREAKDOWN, QCD_EINVAL (m < 0,
  * tol <= 0, maxiter < 0, kinds, missing workspace, x aliases b), QCD_ECUDA.
  * b = 0 gives x = 0, iters = 0, QCD_OK.  Synchronises the stream.
+ * b and x must not overlap each other nor the bound workspace (byte ranges; QCD_EINVAL).
+ * Every entry point that enqueues work returns QCD_EINVAL when the current CUDA device is not the one the context
+ * was created on (qcd_init records cudaGetDevice()).
  */
 qcd_status qcd_cg_solve(qcd_ctx *ctx, const qcd_field *U, const qcd_field *b, qcd_field *x,
                         double m, double tol, int maxiter, qcd_cg_info *info);
@@ -195,7 +200,7 @@ qcd_status qcd_cg_finish(qcd_ctx *ctx, qcd_cg_info *info);
  * recurrence residual CG tests against tol^2 (reading R6).  Recorded on the device by the kernel
  * that advances the recurrence (no extra launch or host round trip during the solve), for the
  * first 16384 iterations of every right-hand side; all three solver loops record it.
- *   rhs      : 0 for qcd_cg_solve; 0 .. n-1 after a multi solve
+ *   rhs      : 0 for qcd_cg_solve; 0 .. n-1 after a multi solve of n right-hand sides (rhs >= n: QCD_EINVAL)
  *   host_out : HOST array of `cap` doubles (may be NULL when cap = 0)
  *   n        : receives min(iters, cap, 16384)
  * Valid from qcd_cg_finish / the return of qcd_cg_solve until the next solve begins on the context
@@ -265,6 +270,15 @@ qcd_status qcd_set_dslash_variant(qcd_ctx *ctx, int variant);
  */
 qcd_status qcd_set_cg_loop(qcd_ctx *ctx, int mode);
 /*
+ * The loop the most recent qcd_cg_solve / qcd_cg_solve_multi / inner solve of qcd_cg_solve_mixed of this context
+ * actually ran: 1, 2 or 3 as above (1 also for a solve driven by qcd_cg_begin / qcd_cg_iterate); 0 before the first
+ * solve or for a NULL context.  With mode 0 this is the library's choice; a FORCED mode that cannot run (2 on the
+ * legacy default stream, 3 with several right-hand sides or without cooperative launch) makes the solve return
+ * QCD_EINVAL instead of falling back, and forced mode 2 still runs kernel by kernel -- reported here as 1 -- while
+ * per-launch profiling is on or when maxiter < 16.
+ */
+int qcd_last_cg_loop(const qcd_ctx *ctx);
+/*
  * Traversal order of the Dslash threads: the sites are walked in
  * chunks of `width` rows of x2 ((x0,x1) fastest, x2 inside the chunk, then x3, then the chunk),
  * which keeps the time-neighbour spinors of several vectors inside the L2.  A pure permutation of
@@ -273,6 +287,21 @@ qcd_status qcd_set_cg_loop(qcd_ctx *ctx, int mode);
  * otherwise a divisor of N2.  Else QCD_EINVAL.
  */
 qcd_status qcd_set_traversal_chunk(qcd_ctx *ctx, int width);
+
+/*
+ * Phase timeline of the persistent solver loop (measurement hook; "global
+ * reductions which have higher latencies ... more pronounced for smaller lattice sizes").
+ *   qcd_cg_timeline_enable(ctx, 1) : solves that run the persistent kernel (qcd_last_cg_loop() == 3) afterwards record, for their
+ *       first 64 iterations, nine %globaltimer stamps (nanoseconds) per iteration in thread 0 of block 0 and of the last block:
+ *       0 phase 1 (p update + D_oe) starts, 1 its work is done, 2 past grid barrier 1, 3 phase 2 (D_eo + M epilogue + block
+ *       partial of <p,Mp>) done, 4 past barrier 2, 5 partials summed / alpha known, 6 phase 3 (x, r update + block partial of
+ *       <r,r>) done, 7 past barrier 3, 8 partials summed / beta known.  0 switches it off (the default; no stamp is taken then).
+ *   qcd_cg_timeline_read : host_out receives [2][n][9] stamps (block 0 first, then the last block), n = min(cap_iters, 64);
+ *       *n_iters = how many of those iterations actually ran.  Synchronises.
+ * Errors: QCD_EINVAL (NULL, solve in progress), QCD_ECUDA.
+ */
+qcd_status qcd_cg_timeline_enable(qcd_ctx *ctx, int on);
+qcd_status qcd_cg_timeline_read(qcd_ctx *ctx, unsigned long long *host_out, int cap_iters, int *n_iters);
 
 /* Re<a,b> over a half-field pair of the same kind (deterministic two-stage reduction,
  * double accumulation); synchronises.  Used by tests and by callers that need norms. */

@@ -33,7 +33,7 @@ SYMBOLS = [
     "qcd_field_download", "qcd_set_workspace", "qcd_dslash_eo", "qcd_dslash_oe", "qcd_apply_M",
     "qcd_cg_solve", "qcd_cg_begin", "qcd_cg_iterate", "qcd_cg_poll", "qcd_cg_finish",
     "qcd_cg_solve_host", "qcd_profile_enable", "qcd_profile_read", "qcd_launch_count",
-    "qcd_set_dslash_variant", "qcd_set_traversal_chunk", "qcd_set_cg_loop", "qcd_re_dot", "qcd_stream_read", "qcd_cg_history",
+    "qcd_set_dslash_variant", "qcd_set_traversal_chunk", "qcd_set_cg_loop", "qcd_last_cg_loop", "qcd_cg_timeline_enable", "qcd_cg_timeline_read", "qcd_re_dot", "qcd_stream_read", "qcd_cg_history",
     # variants and mixed precision
     "qcd_gauge_compress", "qcd_gauge_fix_temporal", "qcd_gauge_set_temporal_unit", "qcd_spinor_rotate",
     "qcd_workspace_bytes_multi", "qcd_dslash_eo_multi", "qcd_dslash_oe_multi", "qcd_cg_solve_multi",
@@ -98,6 +98,9 @@ def load_library() -> ctypes.CDLL:
         "qcd_set_dslash_variant": (ci, [vp, ci]),
         "qcd_set_traversal_chunk": (ci, [vp, ci]),
         "qcd_set_cg_loop": (ci, [vp, ci]),
+        "qcd_last_cg_loop": (ci, [vp]),
+        "qcd_cg_timeline_enable": (ci, [vp, ci]),
+        "qcd_cg_timeline_read": (ci, [vp, P(ctypes.c_ulonglong), ci, P(ci)]),
         "qcd_re_dot": (ci, [vp, vp, vp, P(cd)]),
         "qcd_stream_read": (ci, [vp, vp, ci, P(cd)]),
         "qcd_cg_history": (ci, [vp, ci, P(cd), ci, P(ci)]),
@@ -308,6 +311,21 @@ class Context:
 
     def qcd_set_cg_loop(self, mode: int):
         self._check(self.lib.qcd_set_cg_loop(self.handle, int(mode)), "qcd_set_cg_loop")
+
+    def qcd_last_cg_loop(self) -> int:
+        return int(self.lib.qcd_last_cg_loop(self.handle))
+
+    def qcd_cg_timeline_enable(self, on: bool):
+        self._check(self.lib.qcd_cg_timeline_enable(self.handle, 1 if on else 0), "qcd_cg_timeline_enable")
+
+    def qcd_cg_timeline_read(self, cap_iters: int = 64) -> np.ndarray:
+        """uint64 [2][n][9] %globaltimer stamps (block 0, last block) of the iterations that ran (n <= cap_iters <= 64)."""
+        cap = min(int(cap_iters), 64)
+        out = np.zeros((2, cap, 9), dtype=np.uint64)
+        n = ctypes.c_int()
+        self._check(self.lib.qcd_cg_timeline_read(self.handle, out.ctypes.data_as(ctypes.POINTER(ctypes.c_ulonglong)), cap,
+                                                  ctypes.byref(n)), "qcd_cg_timeline_read")
+        return out[:, : n.value, :].copy()
 
     def qcd_re_dot(self, a: Field, b: Field) -> float:
         r = ctypes.c_double()

@@ -40,7 +40,20 @@ struct PersistArgs {
     T m2;
     double *partials;          // 2 x gridDim.x doubles: [0] Re<p,Ap>, [1] <r,r>
     CgScalars *scal;           // initialised by cg_init_kernel (rr, bb, tol2bb, k, maxiter, flag)
+    unsigned long long *timeline;   // measurement hook (qcd_cg_timeline), NULL in normal solves: %globaltimer stamps of the
+                                    // first TIMELINE_ITERS iterations, [block 0 | last block][iteration][TIMELINE_STAMPS]
 };
+
+// Stamps per iteration: 0 phase 1 starts, 1 phase 1 done, 2 past barrier 1, 3 phase 2 + block partial done, 4 past
+// barrier 2, 5 <p,Ap> summed (alpha known), 6 phase 3 + block partial done, 7 past barrier 3, 8 <r,r> summed (beta known).
+enum { TIMELINE_ITERS = 64, TIMELINE_STAMPS = 9 };
+
+__device__ __forceinline__ unsigned long long global_ns()
+{
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    return t;
+}
 
 __device__ __forceinline__ double2 ld_coherent(const double2 *p) { return __ldcg(p); }
 __device__ __forceinline__ float2 ld_coherent(const float2 *p) { return __ldcg(p); }
@@ -123,8 +136,16 @@ __global__ void __launch_bounds__(PERSIST_BLOCK, 3) cg_persistent_kernel(const P
     int k = a.scal->k, flag = a.scal->flag;
     double alpha = 0.0, beta = 0.0, pAp = 0.0;
 
+    // timeline: thread 0 of block 0 and of the last block stamp the phase boundaries of the first iterations
+    unsigned long long *tl = nullptr;
+    if (a.timeline && threadIdx.x == 0 && (blockIdx.x == 0 || blockIdx.x == gridDim.x - 1))
+        tl = a.timeline + (blockIdx.x == 0 ? 0 : TIMELINE_ITERS * TIMELINE_STAMPS);
+    int it = 0;
+#define QCD_STAMP(i) do { if (tl && it < TIMELINE_ITERS) tl[it * TIMELINE_STAMPS + (i)] = global_ns(); } while (0)
+
     C *p_old = a.p, *p_cur = a.p2;
     while (flag == 0) {
+        QCD_STAMP(0);
         // phase 1: p_cur = r + beta p_old (own even site), t = D_oe p_cur (formed on the fly at the neighbours)
         const T be = (T)beta;
         for (int cb = gtid; cb < Vh; cb += gthreads) {
@@ -145,7 +166,9 @@ __global__ void __launch_bounds__(PERSIST_BLOCK, 3) cg_persistent_kernel(const P
                 p_cur[(size_t)c * sVh + cb] = vp[c];
             }
         }
+        QCD_STAMP(1);
         grid.sync();
+        QCD_STAMP(2);
         // phase 2: Ap = m^2 p - D_eo t, partial Re<p,Ap>
         double dot = 0.0;
         for (int cb = gtid; cb < Vh; cb += gthreads) {
@@ -167,8 +190,11 @@ __global__ void __launch_bounds__(PERSIST_BLOCK, 3) cg_persistent_kernel(const P
             const double s = block_sum<PERSIST_BLOCK>(dot, smem);
             if (threadIdx.x == 0) part_pAp[blockIdx.x] = s;
         }
+        QCD_STAMP(3);
         grid.sync();
+        QCD_STAMP(4);
         pAp = persistent_total(part_pAp, nblocks, smem);
+        QCD_STAMP(5);
         if (!(pAp > 0.0)) { flag = 3; break; }                     // breakdown: uniform across the grid
         alpha = rr / pAp;
         // phase 3: x += alpha p, r -= alpha Ap, partial <r,r>   (elementwise over 3 Vh complex numbers)
@@ -187,8 +213,12 @@ __global__ void __launch_bounds__(PERSIST_BLOCK, 3) cg_persistent_kernel(const P
             const double s = block_sum<PERSIST_BLOCK>(nrm, smem);
             if (threadIdx.x == 0) part_rr[blockIdx.x] = s;
         }
+        QCD_STAMP(6);
         grid.sync();
+        QCD_STAMP(7);
         const double rr_new = persistent_total(part_rr, nblocks, smem);
+        QCD_STAMP(8);
+        ++it;
         beta = rr_new / rr;
         rr = rr_new;
         k += 1;
@@ -202,6 +232,7 @@ __global__ void __launch_bounds__(PERSIST_BLOCK, 3) cg_persistent_kernel(const P
         if (flag != 0) break;
         { C *tmp = p_old; p_old = p_cur; p_cur = tmp; }            // the direction just used becomes "p" of the next update
     }
+#undef QCD_STAMP
     if (gtid == 0) {
         CgScalars *s = a.scal;
         s->rr = rr; s->pAp = pAp; s->alpha = alpha; s->beta = beta; s->k = k; s->flag = flag;

@@ -81,11 +81,11 @@ static cudaError_t launch_staged(const DslashLaunch &d)
     enum { BLOCK = StagedCfg<T, NRHS>::BLOCK, MINB = StagedCfg<T, NRHS>::MINB };
     const size_t smem = (size_t)STAGE_DEPTH * 3 * NROW * BLOCK * sizeof(C);
     auto kernel = dslash_staged_kernel<T, MODE, NROW, TG, NRHS, BLOCK, MINB, STAGE_DEPTH>;
-    static bool configured = false;          // one flag per instantiation
-    if (!configured) {
+    // the attribute belongs to the (function, device) pair: set on every launch (a host-side table update, no device
+    // work) rather than cached per process, which a second device or a second thread would get wrong
+    {
         const cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
-        configured = true;
     }
     DslashArgs<T, NRHS> a;
     a.L = d.L; a.parity = d.parity; a.U = (const C *)d.U;

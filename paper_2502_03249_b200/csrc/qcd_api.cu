@@ -61,6 +61,8 @@ struct qcd_ctx {
     double *d_partials;       // stage-1 partial sums
     unsigned *d_tickets;      // first-level tickets of the two-level last-block election (reduce.cuh)
     double *d_hist;           // residual history, MAXRHS x HIST_CAP (qcd_cg_history)
+    unsigned long long *d_timeline; // phase stamps of the persistent loop, 2 x TIMELINE_ITERS x TIMELINE_STAMPS (qcd_cg_timeline_*)
+    bool timeline_on;
     int partials_cap;
     CgScalars *h_scal;        // pinned, POLL_SLOTS x MAXRHS entries
     cudaEvent_t poll_ev[POLL_SLOTS];
@@ -71,6 +73,9 @@ struct qcd_ctx {
     int variant;
     int chunk;                // Dslash traversal chunk width in x2: 0 = automatic, else a divisor of N2
     int loop;                 // solver loop: 0 automatic, 1 kernel-by-kernel, 2 graph replay, 3 persistent kernel
+    int loop_used;            // loop the most recent qcd_cg_solve* actually ran (qcd_last_cg_loop); 0 = none yet
+    int last_n;               // right-hand sides of the most recent finished solve (qcd_cg_history)
+    int dev;                  // CUDA device the context was created on; every entry point checks it is current
     long long launches;
     // profiling
     bool prof_on;
@@ -96,6 +101,27 @@ static qcd_status fail(qcd_ctx *ctx, qcd_status s, const char *fmt, const char *
         cudaError_t e_ = (call);                                                           \
         if (e_ != cudaSuccess) return fail((ctx), QCD_ECUDA, "%s: %s", #call, cudaGetErrorString(e_)); \
     } while (0)
+
+// The context's allocations, its stream and the occupancy / cooperative-launch queries belong to the device
+// that was current at qcd_init; a call made with another device current would fail late with an opaque CUDA
+// error (or size a cooperative grid from the wrong SM count), so it is rejected here.
+static qcd_status check_device(qcd_ctx *ctx, const char *who)
+{
+    int d = -1;
+    if (cudaGetDevice(&d) != cudaSuccess || d != ctx->dev) {
+        cudaGetLastError();
+        return fail(ctx, QCD_EINVAL, "%s: the current CUDA device is not the one this context was created on (cudaSetDevice first)", who);
+    }
+    return QCD_OK;
+}
+#define DEV(ctx, who) do { const qcd_status ds_ = check_device((ctx), (who)); if (ds_) return ds_; } while (0)
+
+// [a, a + na) and [b, b + nb) share a byte
+static bool overlaps(const void *a, size_t na, const void *b, size_t nb)
+{
+    const uintptr_t a0 = (uintptr_t)a, b0 = (uintptr_t)b;
+    return a0 < b0 + nb && b0 < a0 + na;
+}
 
 extern "C" const char *qcd_strerror(qcd_status s)
 {
@@ -175,13 +201,13 @@ extern "C" qcd_status qcd_init(qcd_ctx **out, const int dims[4], int precision, 
     c->L.s1 = c->L.h; c->L.s2 = c->L.h * dims[1]; c->L.s3 = c->L.h * dims[1] * dims[2];
     c->prec = precision; c->rsize = precision == 64 ? 8 : 4;
     c->stream = (cudaStream_t)cuda_stream;
-    c->variant = 0; c->launches = 0; c->chunk = 0; c->loop = 0;
+    c->variant = 0; c->launches = 0; c->chunk = 0; c->loop = 0; c->loop_used = 0; c->last_n = 0; c->dev = dev;
     c->L.W = dims[2];
     c->prof_on = false; c->prof_created = false; c->prof_n = c->prof_dropped = 0;
     c->ws = nullptr; c->ws_bytes = 0;
     memset(&c->cg, 0, sizeof c->cg);
     c->d_scal = c->d_aux = nullptr; c->d_partials = nullptr; c->d_tickets = nullptr; c->h_scal = nullptr; c->d_stage = nullptr;
-    c->d_hist = nullptr;
+    c->d_hist = nullptr; c->d_timeline = nullptr; c->timeline_on = false;
     for (int i = 0; i < POLL_SLOTS; ++i) c->poll_ev[i] = nullptr;
 
     c->partials_cap = MAXRHS * (dslash_grid_max(c) > blas_grid(c) ? dslash_grid_max(c) : blas_grid(c));
@@ -203,6 +229,9 @@ extern "C" qcd_status qcd_init(qcd_ctx **out, const int dims[4], int precision, 
         err = cudaMemcpy(&c->d_scal[i].hist, &h, sizeof h, cudaMemcpyHostToDevice);
         if (err == cudaSuccess) err = cudaMemcpy(&c->d_scal[i].hist_cap, &cap, sizeof cap, cudaMemcpyHostToDevice);
     }
+    const size_t tl_bytes = 2 * TIMELINE_ITERS * TIMELINE_STAMPS * sizeof(unsigned long long);
+    if (err == cudaSuccess) err = cudaMalloc(&c->d_timeline, tl_bytes);
+    if (err == cudaSuccess) err = cudaMemset(c->d_timeline, 0, tl_bytes);
     if (err == cudaSuccess) err = cudaMalloc(&c->d_stage, STAGE_BYTES);
     if (err == cudaSuccess) err = cudaMallocHost(&c->h_scal, POLL_SLOTS * MAXRHS * sizeof(CgScalars));
     for (int i = 0; i < POLL_SLOTS && err == cudaSuccess; ++i) err = cudaEventCreateWithFlags(&c->poll_ev[i], cudaEventDisableTiming);
@@ -230,6 +259,7 @@ extern "C" qcd_status qcd_finalize(qcd_ctx *c)
     if (c->d_partials) cudaFree(c->d_partials);
     if (c->d_tickets) cudaFree(c->d_tickets);
     if (c->d_hist) cudaFree(c->d_hist);
+    if (c->d_timeline) cudaFree(c->d_timeline);
     if (c->d_stage) cudaFree(c->d_stage);
     if (c->h_scal) cudaFreeHost(c->h_scal);
     delete c;
@@ -346,6 +376,34 @@ extern "C" qcd_status qcd_set_cg_loop(qcd_ctx *ctx, int mode)
     return QCD_OK;
 }
 
+extern "C" int qcd_last_cg_loop(const qcd_ctx *ctx) { return ctx ? ctx->loop_used : 0; }
+
+extern "C" qcd_status qcd_cg_timeline_enable(qcd_ctx *ctx, int on)
+{
+    if (!ctx) return QCD_EINVAL;
+    if (ctx->cg.active) return fail(ctx, QCD_EINVAL, "qcd_cg_timeline_enable: a solve is in progress");
+    ctx->timeline_on = on != 0;
+    return QCD_OK;
+}
+
+extern "C" qcd_status qcd_cg_timeline_read(qcd_ctx *ctx, unsigned long long *host_out, int cap_iters, int *n_iters)
+{
+    if (!ctx) return QCD_EINVAL;
+    if (!host_out || cap_iters < 0 || !n_iters) return fail(ctx, QCD_EINVAL, "qcd_cg_timeline_read: bad argument");
+    if (ctx->cg.active) return fail(ctx, QCD_EINVAL, "qcd_cg_timeline_read: a solve is in progress");
+    DEV(ctx, "qcd_cg_timeline_read");
+    int n = cap_iters < (int)TIMELINE_ITERS ? cap_iters : (int)TIMELINE_ITERS;
+    for (int blk = 0; blk < 2; ++blk)
+        CU(ctx, cudaMemcpyAsync(host_out + (size_t)blk * n * TIMELINE_STAMPS, ctx->d_timeline + (size_t)blk * TIMELINE_ITERS * TIMELINE_STAMPS,
+                                (size_t)n * TIMELINE_STAMPS * sizeof(unsigned long long), cudaMemcpyDeviceToHost, ctx->stream));
+    CU(ctx, cudaStreamSynchronize(ctx->stream));
+    // iterations that ran: the last stamp of an iteration is non-zero
+    int ran = 0;
+    while (ran < n && host_out[(size_t)ran * TIMELINE_STAMPS + TIMELINE_STAMPS - 1] != 0ULL) ++ran;
+    *n_iters = ran;
+    return QCD_OK;
+}
+
 extern "C" qcd_status qcd_set_dslash_variant(qcd_ctx *ctx, int variant)
 {
     if (!ctx) return QCD_EINVAL;
@@ -404,6 +462,7 @@ extern "C" qcd_status qcd_field_upload(qcd_field *f, const void *host)
 {
     if (!f) return QCD_EINVAL;
     if (!host) return fail(f->ctx, QCD_EINVAL, "qcd_field_upload: NULL host pointer");
+    DEV(f->ctx, "qcd_field_upload");
     f->tg = 0;
     return f->ctx->prec == 64 ? transfer_t<double>(f->ctx, f, host, nullptr) : transfer_t<float>(f->ctx, f, host, nullptr);
 }
@@ -412,6 +471,7 @@ extern "C" qcd_status qcd_field_download(const qcd_field *f, void *host)
 {
     if (!f) return QCD_EINVAL;
     if (!host) return fail(f->ctx, QCD_EINVAL, "qcd_field_download: NULL host pointer");
+    DEV(f->ctx, "qcd_field_download");
     return f->ctx->prec == 64 ? transfer_t<double>(f->ctx, f, nullptr, host) : transfer_t<float>(f->ctx, f, nullptr, host);
 }
 
@@ -474,6 +534,7 @@ static qcd_status dslash_public(qcd_ctx *ctx, const qcd_field *U, int n, qcd_fie
                                 int out_parity, const char *who)
 {
     if (!ctx) return QCD_EINVAL;
+    DEV(ctx, who);
     qcd_status s = check_gauge(ctx, U, who);
     if (s) return s;
     if (n < 1 || n > MAXRHS) return fail(ctx, QCD_EINVAL, "%s: n must be 1 .. QCD_MAX_RHS", who);
@@ -484,8 +545,11 @@ static qcd_status dslash_public(qcd_ctx *ctx, const qcd_field *U, int n, qcd_fie
         o[r] = half_ptr(out[r], out_parity);
         i[r] = half_ptr(in[r], 1 - out_parity);
         if (!o[r] || !i[r]) return fail(ctx, QCD_EINVAL, "%s: spinor parity / kind mismatch", who);
-        if (out[r]->ptr == in[r]->ptr) return fail(ctx, QCD_EINVAL, "%s: out must not alias in", who);
-        for (int q = 0; q < r; ++q) if (o[q] == o[r]) return fail(ctx, QCD_EINVAL, "%s: two outputs alias", who);
+    }
+    const size_t hb = half_spinor_bytes(ctx);
+    for (int r = 0; r < n; ++r) {
+        for (int q = 0; q < n; ++q) if (overlaps(o[r], hb, i[q], hb)) return fail(ctx, QCD_EINVAL, "%s: out must not alias in", who);
+        for (int q = 0; q < r; ++q) if (overlaps(o[q], hb, o[r], hb)) return fail(ctx, QCD_EINVAL, "%s: two outputs alias", who);
     }
     return dslash_launch(ctx, 0, U, n, o, i, out_parity, nullptr, 0.0, ctx->d_aux, 0);
 }
@@ -528,6 +592,7 @@ static qcd_status apply_M_raw(qcd_ctx *ctx, const qcd_field *U, void *out, const
 extern "C" qcd_status qcd_apply_M(qcd_ctx *ctx, const qcd_field *U, qcd_field *out_even, const qcd_field *in_even, double m)
 {
     if (!ctx) return QCD_EINVAL;
+    DEV(ctx, "qcd_apply_M");
     qcd_status s = check_gauge(ctx, U, "qcd_apply_M");
     if (s) return s;
     if (!(m >= 0.0)) return fail(ctx, QCD_EINVAL, "qcd_apply_M: m must be >= 0");
@@ -537,7 +602,10 @@ extern "C" qcd_status qcd_apply_M(qcd_ctx *ctx, const qcd_field *U, qcd_field *o
     void *o = half_ptr(out_even, 0);
     const void *i = half_ptr(in_even, 0);
     if (!o || !i) return fail(ctx, QCD_EINVAL, "qcd_apply_M: both spinors must hold even sites");
-    if (o == i) return fail(ctx, QCD_EINVAL, "qcd_apply_M: out must not alias in");
+    const size_t hb = half_spinor_bytes(ctx);
+    if (overlaps(o, hb, i, hb)) return fail(ctx, QCD_EINVAL, "qcd_apply_M: out must not alias in");
+    if (overlaps(o, hb, ctx->ws, ctx->ws_bytes) || overlaps(i, hb, ctx->ws, ctx->ws_bytes))
+        return fail(ctx, QCD_EINVAL, "qcd_apply_M: out and in must not lie inside the bound workspace");
     return apply_M_raw(ctx, U, o, i, m);
 }
 
@@ -550,6 +618,7 @@ extern "C" qcd_status qcd_re_dot(qcd_ctx *ctx, const qcd_field *a, const qcd_fie
     if (!a || !b || !result || a->ctx != ctx || b->ctx != ctx || a->kind != b->kind ||
         (a->kind != QCD_SPINOR_EVEN && a->kind != QCD_SPINOR_ODD))
         return fail(ctx, QCD_EINVAL, "qcd_re_dot: need two half-fields of the same kind");
+    DEV(ctx, "qcd_re_dot");
     {
         LaunchScope ls(ctx, QCD_K_MISC);
         if (ctx->prec == 64)
@@ -570,6 +639,7 @@ extern "C" qcd_status qcd_stream_read(qcd_ctx *ctx, const qcd_field *f, int reps
 {
     if (!ctx) return QCD_EINVAL;
     if (!f || f->ctx != ctx || reps < 1 || !ms_per_pass) return fail(ctx, QCD_EINVAL, "qcd_stream_read: need a field of this context, reps >= 1 and a result pointer");
+    DEV(ctx, "qcd_stream_read");
     const size_t n16 = qcd_field_bytes(ctx, f->kind) / 16;
     const size_t per = (size_t)STREAM_BLOCK * STREAM_LOADS;
     const size_t grid = (n16 + per - 1) / per;
@@ -654,6 +724,7 @@ extern "C" qcd_status qcd_cg_begin_multi(qcd_ctx *ctx, const qcd_field *U, int n
                                          double m, double tol, int maxiter)
 {
     if (!ctx) return QCD_EINVAL;
+    DEV(ctx, "qcd_cg_begin");
     qcd_status s = check_gauge(ctx, U, "qcd_cg_begin");
     if (s) return s;
     if (n < 1 || n > MAXRHS) return fail(ctx, QCD_EINVAL, "qcd_cg: n must be 1 .. QCD_MAX_RHS");
@@ -664,11 +735,18 @@ extern "C" qcd_status qcd_cg_begin_multi(qcd_ctx *ctx, const qcd_field *U, int n
     for (int r = 0; r < n; ++r) {
         if (!b[r] || !x[r] || b[r]->ctx != ctx || x[r]->ctx != ctx || b[r]->kind != QCD_SPINOR_EVEN || x[r]->kind != QCD_SPINOR_EVEN)
             return fail(ctx, QCD_EINVAL, "qcd_cg: b and x must be QCD_SPINOR_EVEN fields of this context");
-        if (b[r]->ptr == x[r]->ptr) return fail(ctx, QCD_EINVAL, "qcd_cg: x must not alias b");
-        for (int q = 0; q < r; ++q) if (x[q]->ptr == x[r]->ptr) return fail(ctx, QCD_EINVAL, "qcd_cg: two solutions alias");
     }
     if (!ctx->ws || ctx->ws_bytes < qcd_workspace_bytes_multi(ctx, n))
         return fail(ctx, QCD_EINVAL, "qcd_cg: workspace missing or smaller than qcd_workspace_bytes_multi (qcd_set_workspace)");
+    // every x against every b (cg_init zeroes x[q] in one blockIdx.y slice while another reads b[r]), x against x,
+    // and both against the workspace the solver writes
+    const size_t hb = half_spinor_bytes(ctx);
+    for (int r = 0; r < n; ++r) {
+        for (int q = 0; q < n; ++q) if (overlaps(x[r]->ptr, hb, b[q]->ptr, hb)) return fail(ctx, QCD_EINVAL, "qcd_cg: x must not alias b");
+        for (int q = 0; q < r; ++q) if (overlaps(x[q]->ptr, hb, x[r]->ptr, hb)) return fail(ctx, QCD_EINVAL, "qcd_cg: two solutions alias");
+        if (overlaps(x[r]->ptr, hb, ctx->ws, ctx->ws_bytes) || overlaps(b[r]->ptr, hb, ctx->ws, ctx->ws_bytes))
+            return fail(ctx, QCD_EINVAL, "qcd_cg: b and x must not lie inside the bound workspace");
+    }
     if (ctx->cg.active) return fail(ctx, QCD_EINVAL, "qcd_cg_begin: a solve is already in progress");
     ctx->cg.U = U; ctx->cg.n = n; ctx->cg.m = m; ctx->cg.tol = tol; ctx->cg.maxiter = maxiter;
     for (int r = 0; r < n; ++r) { ctx->cg.b[r] = b[r]->ptr; ctx->cg.x[r] = x[r]->ptr; }
@@ -676,6 +754,7 @@ extern "C" qcd_status qcd_cg_begin_multi(qcd_ctx *ctx, const qcd_field *U, int n
     s = ctx->prec == 64 ? cg_begin_t<double>(ctx) : cg_begin_t<float>(ctx);
     if (s) return s;
     ctx->cg.active = true;
+    ctx->loop_used = 1;            // qcd_cg_iterate enqueues kernel by kernel; cg_run overrides it
     return QCD_OK;
 }
 
@@ -689,6 +768,7 @@ extern "C" qcd_status qcd_cg_iterate(qcd_ctx *ctx, int n)
 {
     if (!ctx) return QCD_EINVAL;
     if (!ctx->cg.active) return fail(ctx, QCD_EINVAL, "qcd_cg_iterate: no solve in progress");
+    DEV(ctx, "qcd_cg_iterate");
     if (n < 0) return fail(ctx, QCD_EINVAL, "qcd_cg_iterate: n must be >= 0");
     for (int i = 0; i < n; ++i) {
         qcd_status s = ctx->prec == 64 ? cg_iteration_t<double>(ctx) : cg_iteration_t<float>(ctx);
@@ -739,6 +819,7 @@ extern "C" qcd_status qcd_cg_finish_multi(qcd_ctx *ctx, qcd_cg_info *info)
     if (!ctx) return QCD_EINVAL;
     if (!ctx->cg.active) return fail(ctx, QCD_EINVAL, "qcd_cg_finish: no solve in progress");
     ctx->cg.active = false;
+    ctx->last_n = ctx->cg.n;
     CU(ctx, cudaEventRecord(ctx->cg.ev_end, ctx->stream));
     const CgScalars *s;
     qcd_status st = read_scalars(ctx, &s);
@@ -764,7 +845,9 @@ extern "C" qcd_status qcd_cg_finish_multi(qcd_ctx *ctx, qcd_cg_info *info)
 extern "C" qcd_status qcd_cg_history(qcd_ctx *ctx, int rhs, double *host_out, int cap, int *n)
 {
     if (!ctx) return QCD_EINVAL;
-    if (rhs < 0 || rhs >= MAXRHS || cap < 0 || (cap > 0 && !host_out) || !n) return fail(ctx, QCD_EINVAL, "qcd_cg_history: bad argument");
+    if (rhs < 0 || cap < 0 || (cap > 0 && !host_out) || !n) return fail(ctx, QCD_EINVAL, "qcd_cg_history: bad argument");
+    if (rhs >= ctx->last_n) return fail(ctx, QCD_EINVAL, "qcd_cg_history: rhs must be below the number of right-hand sides of the most recent solve");
+    DEV(ctx, "qcd_cg_history");
     if (ctx->cg.active) return fail(ctx, QCD_EINVAL, "qcd_cg_history: a solve is in progress (qcd_cg_finish first)");
     CgScalars s;
     CU(ctx, cudaMemcpyAsync(&ctx->h_scal[0], ctx->d_scal + rhs, sizeof(CgScalars), cudaMemcpyDeviceToHost, ctx->stream));
@@ -809,6 +892,8 @@ static qcd_status cg_persistent_launch(qcd_ctx *c, bool probe_only, bool *ok)
     a.x = (C *)c->cg.x[0]; a.r = (C *)ws_r(c); a.p = (C *)ws_p(c); a.Ap = (C *)ws_Ap(c); a.t = (C *)ws_t(c);
     a.p2 = (C *)ws_at(c, 4, 1, 0);
     a.m2 = (T)(c->cg.m * c->cg.m); a.partials = c->d_partials; a.scal = c->d_scal;
+    a.timeline = c->timeline_on ? c->d_timeline : nullptr;
+    if (c->timeline_on) CU(c, cudaMemsetAsync(c->d_timeline, 0, 2 * TIMELINE_ITERS * TIMELINE_STAMPS * sizeof(unsigned long long), c->stream));
     void *params[] = { &a };
     LaunchScope ls(c, QCD_K_MISC);
     CU(c, cudaLaunchCooperativeKernel((const void *)kernel, dim3(grid), dim3(PERSIST_BLOCK), params, 0, c->stream));
@@ -869,15 +954,24 @@ static cudaGraphExec_t cg_capture_graph(qcd_ctx *ctx)
 static qcd_status cg_run(qcd_ctx *ctx)
 {
     const int maxiter = ctx->cg.maxiter, n = ctx->cg.n;
+    // a FORCED loop that cannot run is an error, not a silent fall-back (the caller could not tell which loop a
+    // test or a bench row exercised); what the automatic choice picked is reported by qcd_last_cg_loop
+    if (ctx->loop == 2 && ctx->stream == nullptr)
+        return fail(ctx, QCD_EINVAL, "qcd_cg: loop 2 (graph replay) needs a context stream other than the legacy default stream");
+    if (ctx->loop == 3 && n != 1)
+        return fail(ctx, QCD_EINVAL, "qcd_cg: loop 3 (persistent kernel) serves one right-hand side");
     if (persistent_wanted(ctx)) {
         bool ok = false;
         const qcd_status s = cg_persistent(ctx, false, &ok);
+        if (!s && ok) ctx->loop_used = 3;
         if (s || ok) return s;              // launched (qcd_cg_finish synchronises and reads the scalars), or failed
+        if (ctx->loop == 3) return fail(ctx, QCD_EINVAL, "qcd_cg: loop 3 (persistent kernel) cannot be launched cooperatively on this device");
     }
     int enq = 0, head = 0, tail = 0, pending = 0, chunk = 8;
     bool first = true;
     cudaGraphExec_t graph = cg_capture_graph(ctx);
     ctx->cg.graph = graph;
+    ctx->loop_used = graph ? 2 : 1;
     if (graph) chunk = GRAPH_ITERS;
     qcd_status result = QCD_OK;
     for (;;) {
@@ -964,6 +1058,7 @@ extern "C" qcd_status qcd_gauge_compress(qcd_ctx *ctx, const qcd_field *U, qcd_f
     if (!ctx) return QCD_EINVAL;
     if (!U || !U12 || U->ctx != ctx || U12->ctx != ctx || U->kind != QCD_GAUGE || U12->kind != QCD_GAUGE_2ROW)
         return fail(ctx, QCD_EINVAL, "qcd_gauge_compress: need a QCD_GAUGE source and a QCD_GAUGE_2ROW destination of this context");
+    DEV(ctx, "qcd_gauge_compress");
     const size_t plane = (size_t)ctx->L.Vh * 2 * ctx->rsize;
     // rows 0 and 1 of link (parity, mu) are its first 6 planes: 8 contiguous 6-plane copies
     for (int pm = 0; pm < 8; ++pm)
@@ -1003,6 +1098,7 @@ extern "C" qcd_status qcd_gauge_fix_temporal(qcd_ctx *ctx, const qcd_field *U, q
         U->kind != QCD_GAUGE || U_fixed->kind != QCD_GAUGE || g->kind != QCD_COLOUR_MATRIX)
         return fail(ctx, QCD_EINVAL, "qcd_gauge_fix_temporal: need QCD_GAUGE U, QCD_GAUGE U_fixed and QCD_COLOUR_MATRIX g of this context");
     if (U->ptr == U_fixed->ptr) return fail(ctx, QCD_EINVAL, "qcd_gauge_fix_temporal: U_fixed must not alias U");
+    DEV(ctx, "qcd_gauge_fix_temporal");
     if (ctx->prec == 64) gauge_fix_t<double>(ctx, U, U_fixed, g); else gauge_fix_t<float>(ctx, U, U_fixed, g);
     CU(ctx, cudaGetLastError());
     U_fixed->tg = 1;
@@ -1015,6 +1111,7 @@ extern "C" qcd_status qcd_spinor_rotate(qcd_ctx *ctx, const qcd_field *g, qcd_fi
     if (!g || !out || !in || g->ctx != ctx || out->ctx != ctx || in->ctx != ctx || g->kind != QCD_COLOUR_MATRIX ||
         !is_spinor_kind(in->kind) || out->kind != in->kind)
         return fail(ctx, QCD_EINVAL, "qcd_spinor_rotate: need a QCD_COLOUR_MATRIX g and two spinor fields of the same kind");
+    DEV(ctx, "qcd_spinor_rotate");
     const int grid = (ctx->L.Vh + 127) / 128;
     for (int par = 0; par < 2; ++par) {
         void *o = half_ptr(out, par);
@@ -1036,6 +1133,7 @@ extern "C" qcd_status qcd_field_convert(qcd_field *dst, const qcd_field *src)
     qcd_ctx *cd = dst->ctx, *cs = src->ctx;
     if (dst->kind != src->kind || cd->prec == cs->prec || memcmp(&cd->L, &cs->L, sizeof(Lattice)) != 0 || cd->stream != cs->stream)
         return fail(cd, QCD_EINVAL, "qcd_field_convert: need the same kind and lattice, different precisions, one stream");
+    DEV(cd, "qcd_field_convert");
     const size_t n = qcd_field_bytes(cs, src->kind) / cs->rsize;
     const int grid = (int)((n + 255) / 256 < 148 * 16 ? (n + 255) / 256 : 148 * 16);
     {
@@ -1084,6 +1182,8 @@ extern "C" qcd_status qcd_cg_solve_mixed(qcd_ctx *c64, qcd_ctx *c32, const qcd_f
         return fail(c64, QCD_EINVAL, "qcd_cg_solve_mixed: need m >= 0, tol > 0, inner_tol > 0, maxiter >= 0, max_outer >= 0");
     if (!c64->ws || !c32->ws) return fail(c64, QCD_EINVAL, "qcd_cg_solve_mixed: both contexts need a workspace (qcd_set_workspace)");
     if (c64->cg.active || c32->cg.active) return fail(c64, QCD_EINVAL, "qcd_cg_solve_mixed: a CG solve is in progress");
+    DEV(c64, "qcd_cg_solve_mixed");
+    if (c32->dev != c64->dev) return fail(c64, QCD_EINVAL, "qcd_cg_solve_mixed: the two contexts live on different devices");
 
     cudaEvent_t e0, e1;
     CU(c64, cudaEventCreate(&e0));

@@ -315,9 +315,60 @@ def test_cg_edge_cases(q):
         ctx.qcd_dslash_oe(fb, fodd, fb)                    # U is not a gauge field
     with pytest.raises(q.QcdError):
         ctx.qcd_apply_M(fU, fb, fb, 0.1)                   # aliasing
+    # a forced solver loop that cannot run is an error, not a silent fall-back (this context is on the legacy default stream)
+    assert ctx.stream.cuda_stream == 0
+    ctx.qcd_set_cg_loop(2)
+    with pytest.raises(q.QcdError) as e:
+        ctx.qcd_cg_solve(fU, fb, fx, 0.1, 1e-8, 100)
+    assert e.value.status == q.QCD_EINVAL and "stream" in str(e.value)
+    ctx.qcd_set_cg_loop(0)
+    info = ctx.qcd_cg_solve(fU, fb, fx, 0.1, 1e-8, 100)    # the context is usable afterwards
+    assert info["iters"] > 0 and ctx.qcd_last_cg_loop() == 3          # 4^4 fits the L2: the library picks the persistent kernel
     ctx.close()
     with pytest.raises(q.QcdError):
         q.Context((4, 4, 5, 4), 64)
+
+
+def test_aliasing_is_checked_on_byte_ranges(q):
+    """Aliasing checks compare byte ranges, not base pointers: a field bound INSIDE another buffer (or inside the
+    workspace the solver writes) is caught; the two halves of one QCD_SPINOR_FULL field are distinct memory and may
+    serve as out and in of one Dslash."""
+    import torch
+    dims = (4, 4, 4, 4)
+    cfg, U, b = qcd_inputs.config_inputs(0)
+    ctx = q.Context(dims, 64, nrhs=2)
+    fU = ctx.field(q.QCD_GAUGE).upload(U)
+    hb = ctx.qcd_field_bytes(q.QCD_SPINOR_EVEN)
+    big = torch.zeros(2 * hb, dtype=torch.uint8, device=ctx.device)
+    f_lo = ctx.field(q.QCD_SPINOR_EVEN, buf=big[:hb])
+    f_mid = ctx.field(q.QCD_SPINOR_EVEN, buf=big[256: 256 + hb])          # overlaps f_lo, different base pointer
+    f_mid_odd = ctx.field(q.QCD_SPINOR_ODD, buf=big[256: 256 + hb])
+    fb = [ctx.field(q.QCD_SPINOR_EVEN).upload(b), ctx.field(q.QCD_SPINOR_EVEN).upload(b)]
+    fx = [ctx.field(q.QCD_SPINOR_EVEN), ctx.field(q.QCD_SPINOR_EVEN)]
+    for call in (lambda: ctx.qcd_cg_solve(fU, f_lo, f_mid, 0.1, 1e-8, 10),
+                 lambda: ctx.qcd_apply_M(fU, f_lo, f_mid, 0.1),
+                 lambda: ctx.qcd_dslash_oe(fU, f_mid_odd, f_lo),
+                 lambda: ctx.qcd_cg_solve_multi(fU, fb, [fx[0], fb[0]], 0.1, 1e-8, 10),     # x[1] aliases b[0]
+                 lambda: ctx.qcd_cg_solve_multi(fU, fb, [f_lo, f_mid], 0.1, 1e-8, 10)):
+        with pytest.raises(q.QcdError) as e:
+            call()
+        assert e.value.status == q.QCD_EINVAL and "alias" in str(e.value)
+    f_ws = ctx.field(q.QCD_SPINOR_EVEN, buf=ctx.ws[hb: 2 * hb])           # a field inside the solver's workspace
+    for call in (lambda: ctx.qcd_cg_solve(fU, fb[0], f_ws, 0.1, 1e-8, 10), lambda: ctx.qcd_cg_solve(fU, f_ws, fx[0], 0.1, 1e-8, 10),
+                 lambda: ctx.qcd_apply_M(fU, f_ws, fb[0], 0.1)):
+        with pytest.raises(q.QcdError) as e:
+            call()
+        assert e.value.status == q.QCD_EINVAL and "workspace" in str(e.value)
+    # one full field as out (even half) and in (odd half): allowed, and equal to the two-field result
+    phi = qcd_inputs.gaussian_spinor(dims, seed=5)
+    full = ctx.field(q.QCD_SPINOR_FULL).upload(phi)
+    ctx.qcd_dslash_eo(fU, full, full)
+    got = full.download()
+    ref = oracle.dslash(dims, U, phi, 0)
+    par = qcd_inputs.site_parity(dims)
+    assert dslash_rel_err(got[par == 0], ref[par == 0]) <= DSLASH_TOL[64]
+    assert np.array_equal(got[par == 1], phi[par == 1])                    # the odd half is untouched
+    ctx.close()
 
 
 # ------------------------------------------------------------------------------------------
@@ -372,6 +423,7 @@ def test_cg_residual_history_matches_oracle(q, loop, prec):
         fb, fx = ctx.field(q.QCD_SPINOR_EVEN).upload(b), ctx.field(q.QCD_SPINOR_EVEN)
         info = ctx.qcd_cg_solve(fU, fb, fx, m, tol, cfg["maxiter"])
         h = ctx.qcd_cg_history()
+        assert ctx.qcd_last_cg_loop() == loop                       # the forced loop is the one that ran, not a fall-back
         assert info["converged"] and len(h) == info["iters"]
         assert h[-1] == info["rel_resid"] ** 2 or abs(np.sqrt(h[-1]) - info["rel_resid"]) <= 1e-15 * info["rel_resid"]
         assert np.all(h[:-1] > tol * tol) and h[-1] <= tol * tol    # stopped at the FIRST iteration below tol
@@ -387,6 +439,9 @@ def test_cg_residual_history_matches_oracle(q, loop, prec):
         assert len(ctx.qcd_cg_history(0, 0)) == 0
         with pytest.raises(q.QcdError):
             ctx.qcd_cg_history(q.QCD_MAX_RHS, 4)
+        with pytest.raises(q.QcdError) as e:
+            ctx.qcd_cg_history(1, 4)                                 # the solve had ONE right-hand side
+        assert e.value.status == q.QCD_EINVAL
         # a solve stopped at maxiter records exactly maxiter entries, equal to the first ones of the full solve
         info7 = ctx.qcd_cg_solve(fU, fb, fx, m, tol, 7)
         h7 = ctx.qcd_cg_history()
@@ -416,6 +471,11 @@ def test_cg_history_multi_rhs(q):
         assert len(h) == infos[i]["iters"] == len(single[i])
         assert np.array_equal(h, single[i])                          # identical arithmetic and reduction order
     assert len(single[1]) == 0
+    with pytest.raises(q.QcdError):
+        ctx.qcd_cg_history(3)                                        # rhs >= n of the solve that just finished
+    ctx.qcd_cg_solve(fU, fb[0], fx[0], m, tol, 5000)
+    with pytest.raises(q.QcdError):
+        ctx.qcd_cg_history(1)                                        # stale entries of the multi solve are not served
     ctx.close()
 
 

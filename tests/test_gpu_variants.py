@@ -416,6 +416,7 @@ def test_cg_graph_replay_matches_plain_loop(q, prec):
             n0 = ctx.qcd_launch_count()
             info = ctx.qcd_cg_solve(fU, fb, fx, m, tol, 10000)
             launches = ctx.qcd_launch_count() - n0
+            assert ctx.qcd_last_cg_loop() == (2 if use_stream else 1)     # the loop that ran is the one this test is about
             res.append((info, fx.download(), launches))
             # maxiter that is not a multiple of the graph length: stops exactly there
             info2 = ctx.qcd_cg_solve(fU, fb, fx, m, 1e-300, 37)
@@ -428,6 +429,39 @@ def test_cg_graph_replay_matches_plain_loop(q, prec):
     _, oinfo = oracle.cg(dims, _rounded(U, prec).astype(x0.dtype), _rounded(b, prec).astype(x0.dtype), m, tol, 10000)
     assert iters_close(i1["iters"], oinfo["iters"])
     assert oracle.true_residual(dims, _rounded(U, prec), _rounded(b, prec), x1.astype(np.complex128), m) <= tol * (1.0 if prec == 64 else 1.5)
+
+
+def test_cg_timeline_hook(q):
+    """qcd_cg_timeline_*: the persistent loop stamps its phase boundaries for the first iterations when asked to, and
+    takes no stamp (and changes no result) otherwise.  Stamps are nanoseconds of one clock: monotone inside an
+    iteration and from one iteration to the next, in both recorded blocks."""
+    dims, m, tol = (8, 8, 8, 8), 0.1, 1e-10
+    U = qcd_inputs.gauge_field(dims, "haar", seed=0)
+    b = qcd_inputs.gaussian_source(dims, seed=1)
+    ctx = q.Context(dims, 64)
+    fU = ctx.field(q.QCD_GAUGE).upload(U)
+    fb, fx = ctx.field(q.QCD_SPINOR_EVEN).upload(b), ctx.field(q.QCD_SPINOR_EVEN)
+    ctx.qcd_set_cg_loop(3)
+    info0 = ctx.qcd_cg_solve(fU, fb, fx, m, tol, 5000)
+    x0 = fx.download()
+    assert ctx.qcd_cg_timeline_read().shape == (2, 0, 9)                 # off by default: nothing recorded
+    ctx.qcd_cg_timeline_enable(True)
+    info1 = ctx.qcd_cg_solve(fU, fb, fx, m, tol, 5000)
+    assert ctx.qcd_last_cg_loop() == 3 and info1["iters"] == info0["iters"] and np.array_equal(fx.download(), x0)
+    tl = ctx.qcd_cg_timeline_read()
+    assert tl.shape == (2, min(64, info1["iters"]), 9)
+    flat = tl.reshape(2, -1).astype(np.int64)
+    assert np.all(np.diff(flat, axis=1) >= 0)
+    per_iter = np.diff(tl[0, :, 0].astype(np.int64))
+    assert 0 < np.median(per_iter) < 1_000_000                            # an 8^4 iteration takes microseconds, not milliseconds
+    assert ctx.qcd_cg_timeline_read(5).shape == (2, 5, 9)
+    info7 = ctx.qcd_cg_solve(fU, fb, fx, m, 1e-300, 7)                     # a shorter solve: exactly its iterations are reported
+    assert info7["iters"] == 7 and ctx.qcd_cg_timeline_read().shape == (2, 7, 9)
+    ctx.qcd_cg_timeline_enable(False)
+    ctx.qcd_set_cg_loop(1)
+    ctx.qcd_cg_solve(fU, fb, fx, m, tol, 5000)                             # another loop records nothing and is unaffected
+    assert np.allclose(fx.download(), x0, rtol=0, atol=1e-9 * np.max(np.abs(x0)))
+    ctx.close()
 
 
 # ------------------------------------------------------------------------------------------
