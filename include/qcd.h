@@ -245,6 +245,12 @@ long long qcd_launch_count(const qcd_ctx *ctx);
  * Errors: QCD_EINVAL (NULL, foreign field, reps < 1), QCD_ECUDA.
  */
 qcd_status qcd_stream_read(qcd_ctx *ctx, const qcd_field *f, int reps, double *ms_per_pass);
+/*
+ * The same for a field that FITS the L2 (the small-lattice regime: 16^4 links = 37.7 MB): `passes` passes over
+ * the field inside ONE launch after a warm-up launch, so that the L2 -> SM rate is timed and not the kernel launch.
+ * *ms_per_pass = launch time / passes.  L1 is bypassed, every pass is L2 traffic.  Errors as qcd_stream_read.
+ */
+qcd_status qcd_stream_read_resident(qcd_ctx *ctx, const qcd_field *f, int passes, double *ms_per_pass);
 
 /*
  * Tuning knob for the Dslash kernels (bench sweeps and A/B tests, Sec. 10):
@@ -278,6 +284,17 @@ qcd_status qcd_set_cg_loop(qcd_ctx *ctx, int mode);
  * per-launch profiling is on or when maxiter < 16.
  */
 int qcd_last_cg_loop(const qcd_ctx *ctx);
+/*
+ * Loop 3 has two launch shapes: lattices of up to 2048 sites per parity (8^4) run as ONE
+ * thread-block cluster of 1 .. 16 CTAs of 512 threads (barrier.cluster and distributed shared memory instead of a
+ * grid-wide barrier through the L2); larger ones as a cooperative grid.  Same arithmetic, same summation orders up to
+ * the shape of the final sum over blocks.
+ *   qcd_last_cg_cluster : CTAs of the cluster the most recent solve ran as; 0 if it ran as a cooperative grid or did not
+ *                         run loop 3.
+ *   qcd_set_cg_cluster  : 0 forbids the cluster shape (A/B measurements and tests), 1 (default) allows it.
+ */
+int qcd_last_cg_cluster(const qcd_ctx *ctx);
+qcd_status qcd_set_cg_cluster(qcd_ctx *ctx, int on);
 /*
  * Traversal order of the Dslash threads: the sites are walked in
  * chunks of `width` rows of x2 ((x0,x1) fastest, x2 inside the chunk, then x3, then the chunk),

@@ -4,12 +4,12 @@
 // At 16^4 one CG iteration of the multi-kernel path is four kernels of 4-14 us, of which ~4 us
 // each are the tail of a reduction (ticket, last block re-reads the partials) and ~1.5 us each a
 // launch gap.  Here ONE cooperative kernel runs the whole solve: every block is resident, the
-// phases of an iteration are separated by grid-wide barriers, and after the barrier EVERY block
-// sums the per-block partials itself in index order -- no last-block serialisation, no host
-// round trip, and alpha, beta, rr, k and the stop decision are bitwise identical in all blocks,
-// so the control flow stays uniform across the grid.
+// phases of an iteration are separated by grid-wide barriers that carry the reduction, and EVERY
+// block ends a barrier with the same sum -- no last-block serialisation, no host round trip, and
+// alpha, beta, rr, k and the stop decision are bitwise identical in all blocks, so the control
+// flow stays uniform across the grid.
 //
-//   phase 1  p' = r + beta p  (each thread for its own even site, into the OTHER p buffer) and
+//   phase 1  p' = r + beta p  (for the own even site, into the OTHER p buffer) and
 //            t  = D_oe p'  with p' formed on the fly at the eight neighbours from r and p: the
 //            direction update needs no pass and no barrier of its own        | grid barrier
 //   phase 2  Ap = m^2 p' - D_eo t;  partial Re<p',Ap> per block               | grid barrier
@@ -20,16 +20,54 @@
 // (p' = fma(beta, p, r) gives the same bits wherever it is evaluated; beta = 0 in the first
 // iteration, where p = r = b.)
 //
+// What the phase timeline showed (qcd_cg_timeline_*, profiles/r02_small_lattice_timeline.md) and what this
+// file does about it:
+//   * up to 12^4 a phase is a chain of L2 round trips (~0.3 us each), not bandwidth: with one thread per
+//     site the 168-register cap makes ptxas walk the four directions one after the other (2.2 us per
+//     Dslash phase at 4^4 ... 12^4 alike).  A site is therefore handled by a QUAD of lanes, one direction
+//     each: every lane issues all the loads of its forward and backward hop at once (one round trip), the
+//     four partial sums meet in two shuffle steps, and lanes 0..2 of the quad finish one colour each;
+//   * a cooperative-groups grid.sync() costs 1.2-1.8 us and the re-read of the per-block partials after it
+//     another 0.4-0.9 us: 6 of the 15.8 us of a 16^4 iteration and of the 11 us of an 8^4 one.  Two hand-written
+//     replacements (every block polling every block's tagged slot, by all threads and by one warp with a 128-byte
+//     line per slot) were SLOWER from 4 blocks on (2.7 us at 4 blocks, 4-5 us at 64, 7-10 us at 340: the polls
+//     of an all-gather grow with the square of the grid) and grid.sync() stays for grids of several clusters.
+//     Lattices of up to 2048 sites per parity (8^4) run as ONE thread-block cluster of up to 16 CTAs x 512
+//     threads (fp64: 256) instead: the barrier is the hardware barrier.cluster (release / acquire at cluster scope), and the
+//     partial sums are exchanged through distributed shared memory -- every CTA stores its partial into every
+//     peer's slot before it arrives and sums the 16 local slots in rank order after the wait.
+//
 // Fields written inside the kernel (p, t, Ap, r, x) are read with L2-coherent loads (ld.global.cg),
-// never through the read-only path; links are read-only and keep it.  The arithmetic per site is
-// that of dslash_kernel (same helpers, same order).
+// never through the read-only path; links are read-only and keep it.
 #pragma once
+
 #include <cooperative_groups.h>
 
 #include "cg_kernels.cuh"
 #include "dslash.cuh"
 
 namespace qcd {
+
+// ------------------------------------------------------------------------------------------
+// cluster primitives (PTX ISA: barrier.cluster, mapa, st.shared::cluster)
+// ------------------------------------------------------------------------------------------
+__device__ __forceinline__ unsigned cluster_ctarank() { unsigned r; asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r)); return r; }
+__device__ __forceinline__ unsigned cluster_nctarank() { unsigned r; asm volatile("mov.u32 %0, %%cluster_nctarank;" : "=r"(r)); return r; }
+// arrive with release, wait with acquire, both at cluster scope: the writes (global and shared) of every thread of the
+// cluster before its arrive are visible to every thread of the cluster after its wait
+__device__ __forceinline__ void cluster_barrier()
+{
+    asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory");
+    asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+// store a double into the shared memory of CTA `rank` of the cluster, at the address that `local` has in this CTA
+__device__ __forceinline__ void st_shared_cluster(double *local, unsigned rank, double v)
+{
+    const unsigned la = (unsigned)__cvta_generic_to_shared(local);
+    unsigned ra;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(ra) : "r"(la), "r"(rank));
+    asm volatile("st.shared::cluster.f64 [%0], %1;" :: "r"(ra), "d"(v) : "memory");
+}
 
 template <typename T>
 struct PersistArgs {
@@ -38,14 +76,15 @@ struct PersistArgs {
     const C *U;
     C *x, *r, *p, *p2, *Ap, *t; // even half-fields (p and p2 alternate as direction vector), t odd
     T m2;
-    double *partials;          // 2 x gridDim.x doubles: [0] Re<p,Ap>, [1] <r,r>
+    double *partials;          // grid version: gridDim.x doubles, the per-block partial sums of the current barrier
     CgScalars *scal;           // initialised by cg_init_kernel (rr, bb, tol2bb, k, maxiter, flag)
-    unsigned long long *timeline;   // measurement hook (qcd_cg_timeline), NULL in normal solves: %globaltimer stamps of the
+    unsigned long long *timeline;   // measurement hook (qcd_cg_timeline_*), NULL in normal solves: %globaltimer stamps of the
                                     // first TIMELINE_ITERS iterations, [block 0 | last block][iteration][TIMELINE_STAMPS]
 };
 
 // Stamps per iteration: 0 phase 1 starts, 1 phase 1 done, 2 past barrier 1, 3 phase 2 + block partial done, 4 past
-// barrier 2, 5 <p,Ap> summed (alpha known), 6 phase 3 + block partial done, 7 past barrier 3, 8 <r,r> summed (beta known).
+// barrier 2 with <p,Ap> summed, 5 alpha known, 6 phase 3 + block partial done, 7 past barrier 3 with <r,r> summed,
+// 8 beta known.
 enum { TIMELINE_ITERS = 64, TIMELINE_STAMPS = 9 };
 
 __device__ __forceinline__ unsigned long long global_ns()
@@ -58,9 +97,60 @@ __device__ __forceinline__ unsigned long long global_ns()
 __device__ __forceinline__ double2 ld_coherent(const double2 *p) { return __ldcg(p); }
 __device__ __forceinline__ float2 ld_coherent(const float2 *p) { return __ldcg(p); }
 
+enum { PERSIST_BLOCK = 128, CLUSTER_MAX_CTAS = 16 };
+// A lane keeps two links and up to four neighbour vectors in flight: 34 sixteen-byte loads = 136 registers in fp64.
+// Under a 168-register cap ptxas interleaves those loads with the FMAs that consume them (four dependent round trips
+// per phase instead of one), so the fp64 kernels run with a 255-register cap: 2 resident blocks of the grid version,
+// 256-thread CTAs in the cluster version (fp32: 4 blocks, 512 threads).
+// Measured (profiles/r02_small_lattice_timeline.md): the quad split halves the fp32 phases (3-5 us -> 1-2.6 us) and
+// is SLOWER in fp64 at every size (a lane's two links and four vectors are 136 registers of loads in flight; ptxas
+// interleaves them with the FMAs under a 168-register cap, and with a 255-register cap the index arithmetic, now
+// done by four lanes per site, fills the issue slots).  fp64 therefore keeps one thread per site (SPLIT = 1).
+template <typename T> struct PersistSplit { enum { value = sizeof(T) == 8 ? 1 : 4 }; };
+template <typename T> struct PersistMinB { enum { value = sizeof(T) == 8 ? 3 : 4 }; };
+template <typename T> struct ClusterBlock { enum { value = sizeof(T) == 8 ? 128 : 512 }; };   // 16 CTAs hold 2048 sites either way
+
+// Barrier of the whole solve's thread set carrying this block's partial sum `block_val` (valid in thread 0; every
+// thread of the block has passed a __syncthreads() after its last global store of the phase -- block_sum provides
+// one).  Returns, in EVERY thread of every block, the sum of all blocks' partials in an order that depends only on
+// the launch shape.
+//   CLUSTER: the solve is one thread-block cluster.  Thread 0 stores the partial into slot [epoch parity][own rank] of
+//            every CTA's shared memory, everybody meets at barrier.cluster, everybody adds the local slots in rank
+//            order.  The parity double-buffers the slots: a CTA cannot write epoch e + 2 before all have read e.
+//   grid   : cooperative launch; partials[block] then cooperative-groups grid.sync(), then every block re-reads all
+//            partials from the L2 and sums them thread-strided and through the block tree.
+template <int BLOCK, bool CLUSTER>
+__device__ __forceinline__ double solve_barrier(double block_val, unsigned epoch, double *partials, double *smem /* BLOCK/32 + 1 */,
+                                                double *cl_slots /* 2 x CLUSTER_MAX_CTAS, shared */)
+{
+    if (CLUSTER) {
+        const unsigned n = cluster_nctarank();
+        double *mine = cl_slots + (epoch & 1u) * CLUSTER_MAX_CTAS;
+        if (threadIdx.x == 0) {
+            const unsigned me = cluster_ctarank();
+            for (unsigned r = 0; r < n; ++r) st_shared_cluster(mine + me, r, block_val);
+        }
+        cluster_barrier();
+        double s = 0.0;
+        for (unsigned r = 0; r < n; ++r) s += mine[r];
+        return s;
+    } else {
+        namespace cg = cooperative_groups;
+        if (threadIdx.x == 0) partials[blockIdx.x] = block_val;
+        cg::this_grid().sync();
+        double s = 0.0;
+        for (int i = threadIdx.x; i < (int)gridDim.x; i += BLOCK) s += __ldcg(partials + i);
+        __syncthreads();                                      // smem is reused
+        const double tot = block_sum<BLOCK>(s, smem);
+        if (threadIdx.x == 0) smem[BLOCK / 32] = tot;
+        __syncthreads();
+        return smem[BLOCK / 32];
+    }
+}
+
 // acc = (D in)(cb) for the site cb of `parity`; `in` may have been written earlier in this kernel
 // FUSE: the input vector is r + beta * in, formed at every neighbour on the fly
-template <typename T, int NROW, int TG, bool FUSE>
+template <typename T, int NROW, int TG, bool FUSE, bool KEEP_L1>
 __device__ __forceinline__ void persistent_site(typename Cplx<T>::type acc[3], const Lattice &L, int parity, int cb,
                                                 const typename Cplx<T>::type *U, const typename Cplx<T>::type *in,
                                                 const typename Cplx<T>::type *r = nullptr, T beta = (T)0)
@@ -77,8 +167,14 @@ __device__ __forceinline__ void persistent_site(typename Cplx<T>::type acc[3], c
         const bool unit_f = TG && mu == 3 && g.x3 != 0;
         const bool unit_b = TG && mu == 3 && g.x3 != 1;
         C uf[9], ub[9], pf[3], pb[3];
-        if (!unit_f) load_link<NROW, C>(uf, Uf + (size_t)(mu * 3 * NROW) * Vh, Vh, pol);
-        if (!unit_b) load_link<NROW, C>(ub, Ub + (size_t)(mu * 3 * NROW) * Vh + g.nb[mu], Vh, pol);
+        if (!unit_f) {
+#pragma unroll
+            for (int k = 0; k < 3 * NROW; ++k) uf[k] = KEEP_L1 ? ld_keep(Uf + (size_t)(mu * 3 * NROW + k) * Vh, pol) : ld_stream(Uf + (size_t)(mu * 3 * NROW + k) * Vh, pol);
+        }
+        if (!unit_b) {
+#pragma unroll
+            for (int k = 0; k < 3 * NROW; ++k) ub[k] = KEEP_L1 ? ld_keep(Ub + (size_t)(mu * 3 * NROW + k) * Vh + g.nb[mu], pol) : ld_stream(Ub + (size_t)(mu * 3 * NROW + k) * Vh + g.nb[mu], pol);
+        }
         const unsigned nf = g.sf[mu] < 0.f ? 1u : 0u, nb = g.sb[mu] < 0.f ? 1u : 0u;
 #pragma unroll
         for (int c = 0; c < 3; ++c) {
@@ -100,34 +196,113 @@ __device__ __forceinline__ void persistent_site(typename Cplx<T>::type acc[3], c
     }
 }
 
-enum { PERSIST_BLOCK = 128 };
-
-// sum of partials[0 .. n) in an order that depends only on n and the block size; the result is
-// returned in EVERY thread of the block (identical in every block of the grid)
-__device__ __forceinline__ double persistent_total(const double *partials, int n, double *smem /* PERSIST_BLOCK/32 + 1 */)
-{
-    double s = 0.0;
-    for (int i = threadIdx.x; i < n; i += PERSIST_BLOCK) s += __ldcg(partials + i);
-    __syncthreads();
-    const double tot = block_sum<PERSIST_BLOCK>(s, smem);
-    if (threadIdx.x == 0) smem[PERSIST_BLOCK / 32] = tot;
-    __syncthreads();
-    return smem[PERSIST_BLOCK / 32];
-}
-
-template <typename T, int NROW, int TG>
-__global__ void __launch_bounds__(PERSIST_BLOCK, 3) cg_persistent_kernel(const PersistArgs<T> a)
+// One direction (forward and backward hop) of (D in)(cb) for the site cb of `parity`: lane mu of a quad.
+// FUSE: the input vector is r + beta * in, formed at both neighbours on the fly.  All loads are issued before
+// the first use.  Same helpers and the same FMA order per hop as dslash_kernel; the four directions are then
+// added as (d0 + d1) + (d2 + d3) by quad_sum (dslash_kernel adds them one after the other).
+template <typename T, int NROW, int TG, bool FUSE, bool KEEP_L1>
+__device__ __forceinline__ void persistent_dir(typename Cplx<T>::type acc[3], const Lattice &L, int parity, int cb, int mu,
+                                               const typename Cplx<T>::type *U, const typename Cplx<T>::type *in,
+                                               const typename Cplx<T>::type *r, T beta)
 {
     typedef typename Cplx<T>::type C;
-    namespace cg = cooperative_groups;
-    cg::grid_group grid = cg::this_grid();
-    __shared__ double smem[PERSIST_BLOCK / 32 + 1];
+    const size_t Vh = (size_t)L.Vh;
+    const unsigned ucb = (unsigned)cb;
+    const int xh = (int)(ucb % (unsigned)L.h);
+    unsigned q = ucb / (unsigned)L.h;
+    const int x1 = (int)(q % (unsigned)L.N1);
+    q /= (unsigned)L.N1;
+    const int x2 = (int)(q % (unsigned)L.N2);
+    const int x3 = (int)(q / (unsigned)L.N2);
+    const int rp = (x1 + x2 + x3 + parity) & 1;           // x0 = 2 xh + rp
+    int nf, nb;
+    if (mu == 0) {
+        nf = rp ? ((xh + 1 == L.h) ? cb - (L.h - 1) : cb + 1) : cb;
+        nb = rp ? cb : ((xh == 0) ? cb + (L.h - 1) : cb - 1);
+    } else {
+        const int xm = mu == 1 ? x1 : (mu == 2 ? x2 : x3);
+        const int Nm = mu == 1 ? L.N1 : (mu == 2 ? L.N2 : L.N3);
+        const int sm = mu == 1 ? L.s1 : (mu == 2 ? L.s2 : L.s3);
+        nf = (xm + 1 == Nm) ? cb - (Nm - 1) * sm : cb + sm;
+        nb = (xm == 0) ? cb + (Nm - 1) * sm : cb - sm;
+    }
+    // eta_mu(x) = (-1)^{x0 + ... + x_{mu-1}}; the forward term carries eta (times -1 across the time seam), the backward
+    // term MINUS eta (R3, R4)
+    const unsigned e = (unsigned)((mu >= 1 ? rp : 0) + (mu >= 2 ? x1 : 0) + (mu >= 3 ? x2 : 0)) & 1u;
+    const unsigned negf = e ^ ((mu == 3 && x3 + 1 == L.N3) ? 1u : 0u);
+    const unsigned negb = (e ^ 1u) ^ ((mu == 3 && x3 == 0) ? 1u : 0u);
+    const bool unit_f = TG && mu == 3 && x3 != 0;
+    const bool unit_b = TG && mu == 3 && x3 != 1;
+
+    const uint64_t pol = l2_policy_evict_last();             // everything is meant to stay in the L2 here
+    const C *Uf = U + (size_t)(parity * 12 * NROW + mu * 3 * NROW) * Vh + cb;
+    const C *Ub = U + (size_t)((1 - parity) * 12 * NROW + mu * 3 * NROW) * Vh + nb;
+    C uf[9], ub[9], pf[3], pb[3], rf[3], rb[3];
+    // KEEP_L1 (one-cluster solves): a CTA handles the same sites in every iteration, so its links may stay in its L1
+    if (!unit_f) {
+#pragma unroll
+        for (int k = 0; k < 3 * NROW; ++k) uf[k] = KEEP_L1 ? ld_keep(Uf + (size_t)k * Vh, pol) : ld_stream(Uf + (size_t)k * Vh, pol);
+    }
+    if (!unit_b) {
+#pragma unroll
+        for (int k = 0; k < 3 * NROW; ++k) ub[k] = KEEP_L1 ? ld_keep(Ub + (size_t)k * Vh, pol) : ld_stream(Ub + (size_t)k * Vh, pol);
+    }
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        pf[c] = ld_coherent(in + (size_t)c * Vh + nf);
+        pb[c] = ld_coherent(in + (size_t)c * Vh + nb);
+        if (FUSE) { rf[c] = ld_coherent(r + (size_t)c * Vh + nf); rb[c] = ld_coherent(r + (size_t)c * Vh + nb); }
+    }
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        if (FUSE) {
+            pf[c].x = fma(beta, pf[c].x, rf[c].x); pf[c].y = fma(beta, pf[c].y, rf[c].y);
+            pb[c].x = fma(beta, pb[c].x, rb[c].x); pb[c].y = fma(beta, pb[c].y, rb[c].y);
+        }
+        pf[c].x = flip_sign(pf[c].x, negf); pf[c].y = flip_sign(pf[c].y, negf);
+        pb[c].x = flip_sign(pb[c].x, negb); pb[c].y = flip_sign(pb[c].y, negb);
+    }
+    if (!unit_f) { if (NROW == 2) reconstruct_third_row<C>(uf); mat_vec_acc<T, C>(acc, uf, pf); } else vec_acc<C>(acc, pf);
+    if (!unit_b) { if (NROW == 2) reconstruct_third_row<C>(ub); matdag_vec_acc<T, C>(acc, ub, pb); } else vec_acc<C>(acc, pb);
+}
+
+// sum over the four lanes of a quad, (l0 + l1) + (l2 + l3); every lane ends with the same bits (fp addition commutes)
+__device__ __forceinline__ double quad_add(double v)
+{
+    v += __shfl_xor_sync(0xffffffffu, v, 1);
+    v += __shfl_xor_sync(0xffffffffu, v, 2);
+    return v;
+}
+__device__ __forceinline__ float quad_add(float v)
+{
+    v += __shfl_xor_sync(0xffffffffu, v, 1);
+    v += __shfl_xor_sync(0xffffffffu, v, 2);
+    return v;
+}
+template <typename C>
+__device__ __forceinline__ C quad_sum_pick(const C acc[3], int lane_in_quad)
+{
+    C a0, a1, a2;
+    a0.x = quad_add(acc[0].x); a0.y = quad_add(acc[0].y);
+    a1.x = quad_add(acc[1].x); a1.y = quad_add(acc[1].y);
+    a2.x = quad_add(acc[2].x); a2.y = quad_add(acc[2].y);
+    return lane_in_quad == 0 ? a0 : (lane_in_quad == 1 ? a1 : a2);     // lane c < 3 finishes colour c
+}
+
+template <typename T, int NROW, int TG, int BLOCK, bool CLUSTER, int SPLIT>
+__device__ __forceinline__ void cg_persistent_body(const PersistArgs<T> &a)
+{
+    static_assert(SPLIT == 1 || SPLIT == 4, "a site is one thread or a quad of lanes");
+    typedef typename Cplx<T>::type C;
+    __shared__ double smem[BLOCK / 32 + 1];
+    __shared__ double cl_slots[2 * CLUSTER_MAX_CTAS];
     const int Vh = a.L.Vh;
     const size_t sVh = (size_t)Vh;
-    const int gthreads = gridDim.x * PERSIST_BLOCK;
-    const int gtid = blockIdx.x * PERSIST_BLOCK + threadIdx.x;
-    const int nblocks = (int)gridDim.x;
-    double *part_pAp = a.partials, *part_rr = a.partials + nblocks;
+    const int gthreads = gridDim.x * BLOCK;
+    const int gtid = blockIdx.x * BLOCK + threadIdx.x;
+    const int nquads = gthreads / SPLIT, quad = gtid / SPLIT, mu = gtid % SPLIT;      // SPLIT = 1: quad = thread, mu = 0
+    unsigned epoch = 0;
+    if (CLUSTER) cluster_barrier();                 // every CTA of the cluster is running before anyone stores into its shared memory
 
     // the recurrence state, replicated: every thread of every block holds the same values
     double rr = a.scal->rr;
@@ -148,77 +323,124 @@ __global__ void __launch_bounds__(PERSIST_BLOCK, 3) cg_persistent_kernel(const P
         QCD_STAMP(0);
         // phase 1: p_cur = r + beta p_old (own even site), t = D_oe p_cur (formed on the fly at the neighbours)
         const T be = (T)beta;
-        for (int cb = gtid; cb < Vh; cb += gthreads) {
-            C acc[3];
-            persistent_site<T, NROW, TG, true>(acc, a.L, 1, cb, a.U, p_old, a.r, be);
-            // all six loads before the first store: one L2 round trip instead of three (a load issued after a
-            // store that may alias it waits for that store)
-            C vp[3], vr[3];
+        for (int s0 = 0; s0 < Vh; s0 += nquads) {               // the same trip count in every thread: the quad shuffles are warp-wide
+            const int cb = s0 + quad;
+            const bool active = cb < Vh;
+            if (SPLIT == 1) {
+                if (active) {
+                    C acc[3];
+                    persistent_site<T, NROW, TG, true, CLUSTER>(acc, a.L, 1, cb, a.U, p_old, a.r, be);
+                    // all six loads before the first store: one L2 round trip instead of three (a load issued after a
+                    // store that may alias it waits for that store)
+                    C vp[3], vr[3];
 #pragma unroll
-            for (int c = 0; c < 3; ++c) {
-                vp[c] = ld_coherent(p_old + (size_t)c * sVh + cb);
-                vr[c] = ld_coherent(a.r + (size_t)c * sVh + cb);
-            }
+                    for (int c = 0; c < 3; ++c) {
+                        vp[c] = ld_coherent(p_old + (size_t)c * sVh + cb);
+                        vr[c] = ld_coherent(a.r + (size_t)c * sVh + cb);
+                    }
 #pragma unroll
-            for (int c = 0; c < 3; ++c) {
-                a.t[(size_t)c * sVh + cb] = acc[c];
-                vp[c].x = fma(be, vp[c].x, vr[c].x); vp[c].y = fma(be, vp[c].y, vr[c].y);
-                p_cur[(size_t)c * sVh + cb] = vp[c];
+                    for (int c = 0; c < 3; ++c) {
+                        a.t[(size_t)c * sVh + cb] = acc[c];
+                        vp[c].x = fma(be, vp[c].x, vr[c].x); vp[c].y = fma(be, vp[c].y, vr[c].y);
+                        p_cur[(size_t)c * sVh + cb] = vp[c];
+                    }
+                }
+            } else {
+                C acc[3], vp, vr;
+                acc[0].x = acc[0].y = acc[1].x = acc[1].y = acc[2].x = acc[2].y = (T)0;
+                vp.x = vp.y = vr.x = vr.y = (T)0;
+                if (active) {
+                    if (mu < 3) {                                // the site-local operands travel with the neighbour loads
+                        vp = ld_coherent(p_old + (size_t)mu * sVh + cb);
+                        vr = ld_coherent(a.r + (size_t)mu * sVh + cb);
+                    }
+                    persistent_dir<T, NROW, TG, true, CLUSTER>(acc, a.L, 1, cb, mu, a.U, p_old, a.r, be);
+                }
+                const C tc = quad_sum_pick<C>(acc, mu);
+                if (active && mu < 3) {
+                    a.t[(size_t)mu * sVh + cb] = tc;
+                    vp.x = fma(be, vp.x, vr.x); vp.y = fma(be, vp.y, vr.y);
+                    p_cur[(size_t)mu * sVh + cb] = vp;
+                }
             }
         }
         QCD_STAMP(1);
-        grid.sync();
+        if (CLUSTER) cluster_barrier();                          // data barrier: t and p_cur are complete everywhere
+        else cooperative_groups::this_grid().sync();
         QCD_STAMP(2);
         // phase 2: Ap = m^2 p - D_eo t, partial Re<p,Ap>
         double dot = 0.0;
-        for (int cb = gtid; cb < Vh; cb += gthreads) {
-            C acc[3];
-            persistent_site<T, NROW, TG, false>(acc, a.L, 0, cb, a.U, a.t);
-            C vv[3];
+        for (int s0 = 0; s0 < Vh; s0 += nquads) {
+            const int cb = s0 + quad;
+            const bool active = cb < Vh;
+            if (SPLIT == 1) {
+                if (active) {
+                    C acc[3], vv[3];
+                    persistent_site<T, NROW, TG, false, CLUSTER>(acc, a.L, 0, cb, a.U, a.t);
 #pragma unroll
-            for (int c = 0; c < 3; ++c) vv[c] = ld_coherent(p_cur + (size_t)c * sVh + cb);
+                    for (int c = 0; c < 3; ++c) vv[c] = ld_coherent(p_cur + (size_t)c * sVh + cb);
 #pragma unroll
-            for (int c = 0; c < 3; ++c) {
-                C o;
-                o.x = fma(a.m2, vv[c].x, -acc[c].x);
-                o.y = fma(a.m2, vv[c].y, -acc[c].y);
-                a.Ap[(size_t)c * sVh + cb] = o;
-                dot += (double)vv[c].x * (double)o.x + (double)vv[c].y * (double)o.y;
+                    for (int c = 0; c < 3; ++c) {
+                        C o;
+                        o.x = fma(a.m2, vv[c].x, -acc[c].x);
+                        o.y = fma(a.m2, vv[c].y, -acc[c].y);
+                        a.Ap[(size_t)c * sVh + cb] = o;
+                        dot += (double)vv[c].x * (double)o.x + (double)vv[c].y * (double)o.y;
+                    }
+                }
+            } else {
+                C acc[3], vv;
+                acc[0].x = acc[0].y = acc[1].x = acc[1].y = acc[2].x = acc[2].y = (T)0;
+                vv.x = vv.y = (T)0;
+                if (active) {
+                    if (mu < 3) vv = ld_coherent(p_cur + (size_t)mu * sVh + cb);
+                    persistent_dir<T, NROW, TG, false, CLUSTER>(acc, a.L, 0, cb, mu, a.U, a.t, nullptr, (T)0);
+                }
+                const C dc = quad_sum_pick<C>(acc, mu);
+                if (active && mu < 3) {
+                    C o;
+                    o.x = fma(a.m2, vv.x, -dc.x);
+                    o.y = fma(a.m2, vv.y, -dc.y);
+                    a.Ap[(size_t)mu * sVh + cb] = o;
+                    dot += (double)vv.x * (double)o.x + (double)vv.y * (double)o.y;
+                }
             }
         }
-        {
-            const double s = block_sum<PERSIST_BLOCK>(dot, smem);
-            if (threadIdx.x == 0) part_pAp[blockIdx.x] = s;
-        }
+        const double dot_block = block_sum<BLOCK>(dot, smem);
         QCD_STAMP(3);
-        grid.sync();
+        pAp = solve_barrier<BLOCK, CLUSTER>(dot_block, ++epoch, a.partials, smem, cl_slots);
         QCD_STAMP(4);
-        pAp = persistent_total(part_pAp, nblocks, smem);
-        QCD_STAMP(5);
         if (!(pAp > 0.0)) { flag = 3; break; }                     // breakdown: uniform across the grid
         alpha = rr / pAp;
-        // phase 3: x += alpha p, r -= alpha Ap, partial <r,r>   (elementwise over 3 Vh complex numbers)
+        QCD_STAMP(5);
+        // phase 3: x += alpha p, r -= alpha Ap, partial <r,r>   (elementwise over 3 Vh complex numbers; four elements
+        // per thread and pass, all loads before the first store: a load behind a store that may alias it waits for it)
         const T al = (T)alpha;
         double nrm = 0.0;
-        for (int i = gtid; i < 3 * Vh; i += gthreads) {
-            C vx = ld_coherent(a.x + i), vr = ld_coherent(a.r + i);
-            const C vp = ld_coherent(p_cur + i), va = ld_coherent(a.Ap + i);
-            vx.x = fma(al, vp.x, vx.x); vx.y = fma(al, vp.y, vx.y);
-            vr.x = fma(-al, va.x, vr.x); vr.y = fma(-al, va.y, vr.y);
-            a.x[i] = vx; a.r[i] = vr;
-            nrm += (double)vr.x * (double)vr.x + (double)vr.y * (double)vr.y;
+        const int n3 = 3 * Vh;
+        for (int i0 = gtid; i0 < n3; i0 += 4 * gthreads) {
+            C vx[4], vr[4], vp[4], va[4];
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                const int i = i0 + j * gthreads;
+                if (i < n3) { vx[j] = ld_coherent(a.x + i); vr[j] = ld_coherent(a.r + i); vp[j] = ld_coherent(p_cur + i); va[j] = ld_coherent(a.Ap + i); }
+            }
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                const int i = i0 + j * gthreads;
+                if (i < n3) {
+                    vx[j].x = fma(al, vp[j].x, vx[j].x); vx[j].y = fma(al, vp[j].y, vx[j].y);
+                    vr[j].x = fma(-al, va[j].x, vr[j].x); vr[j].y = fma(-al, va[j].y, vr[j].y);
+                    a.x[i] = vx[j]; a.r[i] = vr[j];
+                    nrm += (double)vr[j].x * (double)vr[j].x + (double)vr[j].y * (double)vr[j].y;
+                }
+            }
         }
-        {
-            __syncthreads();
-            const double s = block_sum<PERSIST_BLOCK>(nrm, smem);
-            if (threadIdx.x == 0) part_rr[blockIdx.x] = s;
-        }
+        __syncthreads();                                           // smem of the previous barrier has been read by everyone
+        const double nrm_block = block_sum<BLOCK>(nrm, smem);
         QCD_STAMP(6);
-        grid.sync();
+        const double rr_new = solve_barrier<BLOCK, CLUSTER>(nrm_block, ++epoch, a.partials, smem, cl_slots);
         QCD_STAMP(7);
-        const double rr_new = persistent_total(part_rr, nblocks, smem);
-        QCD_STAMP(8);
-        ++it;
         beta = rr_new / rr;
         rr = rr_new;
         k += 1;
@@ -226,6 +448,8 @@ __global__ void __launch_bounds__(PERSIST_BLOCK, 3) cg_persistent_kernel(const P
             double *const hist = a.scal->hist;
             if (hist && k <= a.scal->hist_cap) hist[k - 1] = rr_new;
         }
+        QCD_STAMP(8);
+        ++it;
         if (rr_new != rr_new) flag = 3;
         else if (rr_new <= tol2bb) flag = 1;
         else if (k >= maxiter) flag = 2;
@@ -237,6 +461,21 @@ __global__ void __launch_bounds__(PERSIST_BLOCK, 3) cg_persistent_kernel(const P
         CgScalars *s = a.scal;
         s->rr = rr; s->pAp = pAp; s->alpha = alpha; s->beta = beta; s->k = k; s->flag = flag;
     }
+    if (CLUSTER) cluster_barrier();                 // no CTA exits while a peer may still store into its shared memory
+}
+
+// cooperative launch, any number of co-resident blocks
+template <typename T, int NROW, int TG>
+__global__ void __launch_bounds__(PERSIST_BLOCK, PersistMinB<T>::value) cg_persistent_kernel(const PersistArgs<T> a)
+{
+    cg_persistent_body<T, NROW, TG, PERSIST_BLOCK, false, PersistSplit<T>::value>(a);
+}
+
+// ONE cluster of 1 .. 16 CTAs (cluster dimension = grid dimension, set at launch)
+template <typename T, int NROW, int TG>
+__global__ void __launch_bounds__(ClusterBlock<T>::value, 1) cg_cluster_kernel(const PersistArgs<T> a)
+{
+    cg_persistent_body<T, NROW, TG, ClusterBlock<T>::value, true, PersistSplit<T>::value>(a);
 }
 
 } // namespace qcd

@@ -28,4 +28,28 @@ __global__ void __launch_bounds__(STREAM_BLOCK) stream_read_kernel(const double2
     if (x == 0xfff7a5a5deadbeefULL) *sink = v[0];
 }
 
+// The same loads over a field that FITS the L2, `passes` times inside ONE launch (grid-stride; a launch per pass
+// would time the launch, not the L2, at 16^4): the denominator of the small-lattice kernels, whose operands are
+// served by the L2 and not by HBM.  L1 is bypassed (no_allocate), so every pass is L2 -> SM traffic.
+__global__ void __launch_bounds__(STREAM_BLOCK) stream_read_resident_kernel(const double2 *__restrict__ p, size_t n16, int passes, double2 *sink)
+{
+    const uint64_t pol = l2_policy_evict_last();
+    const size_t stride = (size_t)gridDim.x * (STREAM_BLOCK * STREAM_LOADS);
+    unsigned long long x = 0;
+    for (int pass = 0; pass < passes; ++pass) {
+        for (size_t base = (size_t)blockIdx.x * (STREAM_BLOCK * STREAM_LOADS) + threadIdx.x; base < n16; base += stride) {
+            double2 v[STREAM_LOADS];
+#pragma unroll
+            for (int k = 0; k < STREAM_LOADS; ++k) {
+                const size_t i = base + (size_t)k * STREAM_BLOCK;
+                v[k] = i < n16 ? ld_stream(p + i, pol) : make_double2(0.0, 0.0);
+            }
+#pragma unroll
+            for (int k = 0; k < STREAM_LOADS; ++k)
+                x ^= (unsigned long long)__double_as_longlong(v[k].x) ^ (unsigned long long)__double_as_longlong(v[k].y);
+        }
+    }
+    if (x == 0xfff7a5a5deadbeefULL) *sink = make_double2(0.0, 0.0);
+}
+
 } // namespace qcd

@@ -73,6 +73,8 @@ struct qcd_ctx {
     int variant;
     int chunk;                // Dslash traversal chunk width in x2: 0 = automatic, else a divisor of N2
     int loop;                 // solver loop: 0 automatic, 1 kernel-by-kernel, 2 graph replay, 3 persistent kernel
+    int persist_cluster;      // CTAs of the cluster the most recent persistent solve ran as, 0 = cooperative grid (qcd_last_cg_cluster)
+    bool loop_cluster_ok;     // the one-cluster form of the persistent loop may be used (qcd_set_cg_cluster; default on)
     int loop_used;            // loop the most recent qcd_cg_solve* actually ran (qcd_last_cg_loop); 0 = none yet
     int last_n;               // right-hand sides of the most recent finished solve (qcd_cg_history)
     int dev;                  // CUDA device the context was created on; every entry point checks it is current
@@ -201,7 +203,7 @@ extern "C" qcd_status qcd_init(qcd_ctx **out, const int dims[4], int precision, 
     c->L.s1 = c->L.h; c->L.s2 = c->L.h * dims[1]; c->L.s3 = c->L.h * dims[1] * dims[2];
     c->prec = precision; c->rsize = precision == 64 ? 8 : 4;
     c->stream = (cudaStream_t)cuda_stream;
-    c->variant = 0; c->launches = 0; c->chunk = 0; c->loop = 0; c->loop_used = 0; c->last_n = 0; c->dev = dev;
+    c->variant = 0; c->launches = 0; c->chunk = 0; c->loop = 0; c->loop_used = 0; c->last_n = 0; c->dev = dev; c->persist_cluster = 0; c->loop_cluster_ok = true;
     c->L.W = dims[2];
     c->prof_on = false; c->prof_created = false; c->prof_n = c->prof_dropped = 0;
     c->ws = nullptr; c->ws_bytes = 0;
@@ -377,6 +379,15 @@ extern "C" qcd_status qcd_set_cg_loop(qcd_ctx *ctx, int mode)
 }
 
 extern "C" int qcd_last_cg_loop(const qcd_ctx *ctx) { return ctx ? ctx->loop_used : 0; }
+
+extern "C" int qcd_last_cg_cluster(const qcd_ctx *ctx) { return (ctx && ctx->loop_used == 3) ? ctx->persist_cluster : 0; }
+
+extern "C" qcd_status qcd_set_cg_cluster(qcd_ctx *ctx, int on)
+{
+    if (!ctx) return QCD_EINVAL;
+    ctx->loop_cluster_ok = on != 0;
+    return QCD_OK;
+}
 
 extern "C" qcd_status qcd_cg_timeline_enable(qcd_ctx *ctx, int on)
 {
@@ -664,6 +675,43 @@ extern "C" qcd_status qcd_stream_read(qcd_ctx *ctx, const qcd_field *f, int reps
     return QCD_OK;
 }
 
+// L2-resident variant: `passes` passes over the field inside ONE launch (measure_kernels.cuh).
+extern "C" qcd_status qcd_stream_read_resident(qcd_ctx *ctx, const qcd_field *f, int passes, double *ms_per_pass)
+{
+    if (!ctx) return QCD_EINVAL;
+    if (!f || f->ctx != ctx || passes < 1 || !ms_per_pass) return fail(ctx, QCD_EINVAL, "qcd_stream_read_resident: need a field of this context, passes >= 1 and a result pointer");
+    DEV(ctx, "qcd_stream_read_resident");
+    const size_t n16 = qcd_field_bytes(ctx, f->kind) / 16;
+    const size_t per = (size_t)STREAM_BLOCK * STREAM_LOADS;
+    int sms = 0;
+    CU(ctx, cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, ctx->dev));
+    size_t grid = (n16 + per - 1) / per;
+    if (grid > (size_t)sms * 8) grid = (size_t)sms * 8;          // 8 resident blocks of 256 threads per SM
+    cudaEvent_t e0, e1;
+    CU(ctx, cudaEventCreate(&e0));
+    CU(ctx, cudaEventCreate(&e1));
+    cudaError_t err = cudaSuccess;
+    {
+        LaunchScope ls(ctx, QCD_K_MISC);                          // warm-up: brings the field into the L2
+        stream_read_resident_kernel<<<(unsigned)grid, STREAM_BLOCK, 0, ctx->stream>>>((const double2 *)f->ptr, n16, 2, (double2 *)ctx->d_stage);
+    }
+    err = cudaEventRecord(e0, ctx->stream);
+    {
+        LaunchScope ls(ctx, QCD_K_MISC);
+        stream_read_resident_kernel<<<(unsigned)grid, STREAM_BLOCK, 0, ctx->stream>>>((const double2 *)f->ptr, n16, passes, (double2 *)ctx->d_stage);
+    }
+    if (err == cudaSuccess) err = cudaGetLastError();
+    if (err == cudaSuccess) err = cudaEventRecord(e1, ctx->stream);
+    if (err == cudaSuccess) err = cudaEventSynchronize(e1);
+    float ms = 0.f;
+    if (err == cudaSuccess) err = cudaEventElapsedTime(&ms, e0, e1);
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    if (err != cudaSuccess) return fail(ctx, QCD_ECUDA, "qcd_stream_read_resident: %s", cudaGetErrorString(err));
+    *ms_per_pass = (double)ms / passes;
+    return QCD_OK;
+}
+
 // ------------------------------------------------------------------------------------------
 // CG (n right-hand sides in lock step; qcd_cg_solve is n = 1)
 // ------------------------------------------------------------------------------------------
@@ -871,32 +919,70 @@ extern "C" qcd_status qcd_cg_finish(qcd_ctx *ctx, qcd_cg_info *info)
 }
 
 // Lattices that fit the L2: the whole solve in ONE cooperative kernel (cg_persistent.cuh).
-enum { PERSIST_MAX_BYTES = 96 << 20 };
+enum { PERSIST_MAX_BYTES = 96 << 20, CLUSTER_MAX_SITES = 2048 };
 
 template <typename T, int NROW, int TG>
 static qcd_status cg_persistent_launch(qcd_ctx *c, bool probe_only, bool *ok)
 {
     typedef typename Cplx<T>::type C;
-    auto kernel = cg_persistent_kernel<T, NROW, TG>;
-    int per_sm = 0, dev = 0, sms = 0, coop = 0;
-    CU(c, cudaGetDevice(&dev));
-    CU(c, cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev));
-    CU(c, cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
-    CU(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, PERSIST_BLOCK, 0));
-    *ok = coop && per_sm > 0;
-    if (probe_only || !*ok) return QCD_OK;
-    int grid = (c->L.Vh + PERSIST_BLOCK - 1) / PERSIST_BLOCK;
-    if (grid > per_sm * sms) grid = per_sm * sms;
     PersistArgs<T> a;
     a.L = c->L; a.U = (const C *)c->cg.U->ptr;
     a.x = (C *)c->cg.x[0]; a.r = (C *)ws_r(c); a.p = (C *)ws_p(c); a.Ap = (C *)ws_Ap(c); a.t = (C *)ws_t(c);
     a.p2 = (C *)ws_at(c, 4, 1, 0);
     a.m2 = (T)(c->cg.m * c->cg.m); a.partials = c->d_partials; a.scal = c->d_scal;
     a.timeline = c->timeline_on ? c->d_timeline : nullptr;
+    enum { SPLIT = PersistSplit<T>::value };                     // lanes per site (cg_persistent.cuh)
+    const int wanted_threads = SPLIT * c->L.Vh;
+
+    // up to 2048 sites per parity: ONE thread-block cluster (hardware barrier, partial sums through DSMEM)
+    enum { CLUSTER_BLOCK = ClusterBlock<T>::value };
+    if (c->L.Vh <= CLUSTER_MAX_SITES && c->loop_cluster_ok) {
+        auto kernel = cg_cluster_kernel<T, NROW, TG>;
+        int ncta = 1;
+        while (ncta * CLUSTER_BLOCK < wanted_threads && ncta < CLUSTER_MAX_CTAS) ncta *= 2;
+        cudaLaunchConfig_t cfg;
+        memset(&cfg, 0, sizeof cfg);
+        cfg.gridDim = dim3(ncta); cfg.blockDim = dim3(CLUSTER_BLOCK); cfg.dynamicSmemBytes = 0; cfg.stream = c->stream;
+        cudaLaunchAttribute attr[1];
+        attr[0].id = cudaLaunchAttributeClusterDimension;
+        attr[0].val.clusterDim.x = ncta; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+        cfg.attrs = attr; cfg.numAttrs = 1;
+        cudaError_t e = cudaSuccess;
+        if (ncta > 8) e = cudaFuncSetAttribute(kernel, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
+        int nclusters = 0;
+        if (e == cudaSuccess) e = cudaOccupancyMaxActiveClusters(&nclusters, kernel, &cfg);
+        if (e == cudaSuccess && nclusters >= 1) {
+            *ok = true;
+            if (probe_only) return QCD_OK;
+            if (c->timeline_on) CU(c, cudaMemsetAsync(c->d_timeline, 0, 2 * TIMELINE_ITERS * TIMELINE_STAMPS * sizeof(unsigned long long), c->stream));
+            LaunchScope ls(c, QCD_K_MISC);
+            CU(c, cudaLaunchKernelEx(&cfg, kernel, a));
+            c->persist_cluster = ncta;
+            return QCD_OK;
+        }
+        cudaGetLastError();                                     // no cluster of that size on this device: the grid version below
+    }
+
+    auto kernel = cg_persistent_kernel<T, NROW, TG>;
+    int per_sm = 0, sms = 0, coop = 0;
+    CU(c, cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, c->dev));
+    CU(c, cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, c->dev));
+    CU(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, PERSIST_BLOCK, 0));
+    *ok = coop && per_sm > 0;
+    if (probe_only || !*ok) return QCD_OK;
+    // at most what is co-resident; when the sites need several passes the grid is shrunk so that the passes are equally full
+    int max_grid = per_sm * sms;
+    if (max_grid * MAXRHS > c->partials_cap) max_grid = c->partials_cap / MAXRHS;
+    const int quads_per_block = PERSIST_BLOCK / SPLIT;
+    const int passes = (c->L.Vh + max_grid * quads_per_block - 1) / (max_grid * quads_per_block);
+    const int per_pass = (c->L.Vh + passes - 1) / passes;
+    int grid = (per_pass + quads_per_block - 1) / quads_per_block;
+    if (grid > max_grid) grid = max_grid;
     if (c->timeline_on) CU(c, cudaMemsetAsync(c->d_timeline, 0, 2 * TIMELINE_ITERS * TIMELINE_STAMPS * sizeof(unsigned long long), c->stream));
     void *params[] = { &a };
     LaunchScope ls(c, QCD_K_MISC);
     CU(c, cudaLaunchCooperativeKernel((const void *)kernel, dim3(grid), dim3(PERSIST_BLOCK), params, 0, c->stream));
+    c->persist_cluster = 0;
     return QCD_OK;
 }
 

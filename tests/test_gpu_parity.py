@@ -391,6 +391,13 @@ def test_stream_read_hook(q, prec):
     assert np.array_equal(fU.download(), U)
     with pytest.raises(q.QcdError):
         ctx.qcd_stream_read(fU, 0)
+    # the L2-resident form: `passes` passes inside ONE launch (after one warm-up launch)
+    n0 = ctx.qcd_launch_count()
+    assert ctx.qcd_stream_read_resident(fU, 7) > 0.0 and ctx.qcd_stream_read_resident(fe, 1) > 0.0
+    assert ctx.qcd_launch_count() - n0 == 4
+    assert np.array_equal(fU.download(), U)
+    with pytest.raises(q.QcdError):
+        ctx.qcd_stream_read_resident(fU, 0)
     other = q.Context(dims, prec)
     with pytest.raises(q.QcdError):
         other.qcd_stream_read(fU, 1)

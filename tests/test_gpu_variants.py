@@ -431,6 +431,53 @@ def test_cg_graph_replay_matches_plain_loop(q, prec):
     assert oracle.true_residual(dims, _rounded(U, prec), _rounded(b, prec), x1.astype(np.complex128), m) <= tol * (1.0 if prec == 64 else 1.5)
 
 
+@pytest.mark.parametrize("prec", [64, 32])
+@pytest.mark.parametrize("dims,links,eps", [((4, 4, 4, 4), "haar", None), ((8, 4, 6, 10), "near_identity", 0.5),
+                                            ((4, 6, 2, 8), "haar", None), ((8, 8, 8, 8), "haar", None)])
+def test_cg_persistent_cluster_and_grid_shapes_agree(q, dims, links, eps, prec):
+    """Loop 3 runs lattices of up to 2048 sites per parity as ONE thread-block cluster (barrier.cluster, partial sums
+    through distributed shared memory) and larger ones as a cooperative grid.  Same
+    per-site arithmetic; only the shape of the final sum over blocks differs.  Both shapes must match the oracle,
+    agree with each other to rounding, and be bitwise reproducible; the library must say which one ran."""
+    m = 0.1
+    tol = 1e-10 if prec == 64 else 1e-5
+    U = qcd_inputs.gauge_field(dims, links, seed=0, eps=eps)
+    b = qcd_inputs.gaussian_source(dims, seed=1)
+    Ur, br = _rounded(U, prec), _rounded(b, prec)
+    ctx = q.Context(dims, prec)
+    fU = ctx.field(q.QCD_GAUGE).upload(U)
+    fb, fx = ctx.field(q.QCD_SPINOR_EVEN).upload(b), ctx.field(q.QCD_SPINOR_EVEN)
+    ctx.qcd_set_cg_loop(3)
+    out = {}
+    for cluster in (True, False):
+        ctx.qcd_set_cg_cluster(cluster)
+        info = ctx.qcd_cg_solve(fU, fb, fx, m, tol, 20000)
+        x = fx.download()
+        assert ctx.qcd_last_cg_loop() == 3
+        ncta = ctx.qcd_last_cg_cluster()
+        assert (1 <= ncta <= 16) if cluster else ncta == 0, ncta
+        info2 = ctx.qcd_cg_solve(fU, fb, fx, m, tol, 20000)
+        assert info2["iters"] == info["iters"] and np.array_equal(fx.download(), x)          # bitwise reproducible
+        out[cluster] = (info, x.astype(np.complex128))
+    (ic, xc), (ig, xg) = out[True], out[False]
+    assert ic["converged"] and ig["converged"] and abs(ic["iters"] - ig["iters"]) <= 1
+    xo, oinfo = oracle.cg(dims, Ur.astype(ctx.cdtype), br.astype(ctx.cdtype), m, tol, 20000)
+    for info, x in (out[True], out[False]):
+        assert iters_close(info["iters"], oinfo["iters"]), (info, oinfo)
+        true = oracle.true_residual(dims, Ur, br, x, m)
+        if prec == 64:
+            assert true <= tol, true
+        else:
+            assert true <= 2.0 * max(tol, oracle.true_residual(dims, Ur, br, xo.astype(np.complex128), m)), true
+    if prec == 64:
+        assert np.linalg.norm(xc - xg) <= 1e-9 * np.linalg.norm(xg)
+    # exact stop at maxiter and the residual history in the cluster shape
+    ctx.qcd_set_cg_cluster(True)
+    info7 = ctx.qcd_cg_solve(fU, fb, fx, m, 1e-300, 7)
+    assert info7["iters"] == 7 and info7["status"] == q.QCD_ENOTCONVERGED and len(ctx.qcd_cg_history()) == 7
+    ctx.close()
+
+
 def test_cg_timeline_hook(q):
     """qcd_cg_timeline_*: the persistent loop stamps its phase boundaries for the first iterations when asked to, and
     takes no stamp (and changes no result) otherwise.  Stamps are nanoseconds of one clock: monotone inside an
