@@ -94,7 +94,10 @@ def parse_args(argv=None):
                     help="run only the Dslash variant sweep (two-row / temporal gauge / NMULTI) and print it; used for ncu captures")
     ap.add_argument("--dslash-only", action="store_true",
                     help="run only `--reps` D_oe and D_eo launches of BASELINE.json configs[--config] in --prec; used for ncu captures")
-    ap.add_argument("--config", type=int, default=4, choices=(0, 1, 2, 3, 4), help="BASELINE.json config of --dslash-only")
+    ap.add_argument("--cg-only", action="store_true",
+                    help="run only `--reps` full CG solves of BASELINE.json configs[--config] in --prec with the solver loop the "
+                         "library picks; used for ncu captures of the small-lattice loops")
+    ap.add_argument("--config", type=int, default=4, choices=(0, 1, 2, 3, 4), help="BASELINE.json config of --dslash-only / --cg-only")
     ap.add_argument("--prec", type=int, default=64, choices=(64, 32),
                     help="precision of --variants-only / --dslash-only, and of the timed CG iterations (32: the fp32 path of "
                          "the same workload, reported with dtype f32 and without the extra reports; the default line is fp64)")
@@ -201,7 +204,7 @@ def free_port() -> int:
 def respawn_under_torchrun(args, argv) -> int | None:
     """`python bench.py --gpus N` with N > 1 and no torchrun environment: launch N ranks (one per GPU) of this very
     command under torch.distributed.run and return its exit code; None when no re-launch is needed."""
-    if args.gpus <= 1 or "WORLD_SIZE" in os.environ or args.variants_only or args.dslash_only:
+    if args.gpus <= 1 or "WORLD_SIZE" in os.environ or args.variants_only or args.dslash_only or args.cg_only:
         return None
     cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(args.gpus),
            "--master-addr", "127.0.0.1", "--master-port", str(free_port()), os.path.abspath(__file__)] + list(argv)
@@ -414,14 +417,16 @@ def run_ours(args):
     side.update({"kernel_ms": kernel_ms, "setup_seconds": round(t_setup, 1), "lattice": list(dims), "sites": V,
                  "bytes_per_even_site_per_step": REALS_ITER_NOMINAL * rsize})
 
-    if rank == 0 and not args.quick and prec == 64:
+    ran_reports = rank == 0 and not args.quick and prec == 64
+    if ran_reports:
         import bench_reports
         bench_reports.run_all(args, q, torch, ctx, out, side, cfg, dims, U, b, hb, hx, fU, fb, fx, fo, peak, stream_gbs)
     del hb, hx
     if rank == 0:
-        path = write_sidecar(args.extras or DEFAULT_EXTRAS, side)
-        if path:
-            out["extras"] = path
+        if ran_reports or args.extras:                    # --quick has nothing beyond the headline and must not overwrite a sidecar
+            path = write_sidecar(args.extras or DEFAULT_EXTRAS, side)
+            if path:
+                out["extras"] = path
         print(headline_line(out), flush=True)
     try:
         ctx.close()
@@ -511,6 +516,30 @@ def run_dslash_only(args):
     ctx.close()
 
 
+def run_cg_only(args):
+    """`--reps` full solves at BASELINE.json configs[--config] (tolerance of that config and precision): the command the
+    captures of the solver-loop kernels under profiles/ are taken with."""
+    import torch
+    import qcd_inputs
+    import paper_2502_03249_b200 as q
+    cfg, U, b = qcd_inputs.config_inputs(args.config)
+    dims = cfg["dims"]
+    tol = cfg["tol64"] if args.prec == 64 else (cfg["tol32"] or 1e-5)
+    stream = torch.cuda.Stream()
+    with torch.cuda.stream(stream):
+        ctx = q.Context(dims, args.prec, stream=stream)
+        fU = ctx.field(q.QCD_GAUGE).upload(U)
+        fb, fx = ctx.field(q.QCD_SPINOR_EVEN).upload(b), ctx.field(q.QCD_SPINOR_EVEN)
+        infos = [ctx.qcd_cg_solve(fU, fb, fx, cfg["m"], tol, cfg["maxiter"]) for _ in range(max(args.reps, 1))]
+        best = min(infos, key=lambda i: i["seconds"])
+        print(json.dumps({"cg_only": True, "config": args.config, "lattice": list(dims), "prec": args.prec, "tol": tol,
+                          "loop": ctx.qcd_last_cg_loop(), "cluster_ctas": ctx.qcd_last_cg_cluster(), "iters": best["iters"],
+                          "converged": best["converged"], "s_per_solve": best["seconds"],
+                          "us_per_iter": round(1e6 * best["seconds"] / max(best["iters"], 1), 3),
+                          "gpu_launches": ctx.qcd_launch_count()}), flush=True)
+        ctx.close()
+
+
 def main(argv=None):
     argv = sys.argv[1:] if argv is None else argv
     args = parse_args(argv)
@@ -521,6 +550,8 @@ def main(argv=None):
         run_variants_only(args)
     elif args.dslash_only:
         run_dslash_only(args)
+    elif args.cg_only:
+        run_cg_only(args)
     elif args.impl == "reference":
         run_reference(args)
     else:

@@ -260,6 +260,9 @@ qcd_status qcd_stream_read_resident(qcd_ctx *ctx, const qcd_field *f, int passes
  *   1, 2, 3 : one-vector kernel with 64 x 8, 256 x 2, 128 x 3 threads x resident blocks
  *   4 : force the staged kernel (links prefetched through shared memory by cp.async)
  *   5 : force the register kernel
+ *   6, 7 : force the pair kernel (two adjacent lanes per site, half of the vectors each, the link shared through the
+ *       cp.async ring) under a 168- / 128-register cap; applies to an even number of vectors >= 4 on a volume of whole
+ *       64-site blocks, otherwise the library's choice runs
  * Every variant computes the same result (bitwise).  Unknown variants -> QCD_EINVAL.
  */
 qcd_status qcd_set_dslash_variant(qcd_ctx *ctx, int variant);

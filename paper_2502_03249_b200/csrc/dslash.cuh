@@ -447,4 +447,154 @@ __global__ void __launch_bounds__(BLOCK, MINB) dslash_staged_kernel(const Dslash
     dslash_reduce<T, MODE, NRHS, BLOCK>(a, dot);
 }
 
+// ------------------------------------------------------------------------------------------
+// Pair variant for an even number of vectors (NRHS = 4, 6, 8): a site is handled by TWO adjacent lanes,
+// each with NRHS / 2 of the vectors.  What it is for (profiles/README.md "n >= 3"): with all
+// NRHS accumulator sets in one thread the register file allows 8 warps per SM and no second set of neighbour
+// vectors, so every hop exposes the L2 latency of its vector loads (one-thread staged kernel: PIPE only up to
+// n = 4 in fp64).  Halving the vectors per thread halves accumulators AND vector registers: the next hop's vectors
+// are requested before the current hop is computed at every n, under a 168-register cap (12 warps).
+// The link is shared through the cp.async ring of the staged kernel: the two lanes copy alternate planes of
+// the link into the pair's column, meet at a __syncwarp() after their own cp.async.wait_group, and both read all
+// planes (same address: a shared-memory broadcast).  A second __syncwarp() before a column is refilled keeps the
+// partner's reads ahead of the overwrite.  No block barrier.  Per vector the FMAs and their order are those of the
+// other kernels: results are bitwise identical.  Needs Vh % (BLOCK / 2) == 0 (the host checks).
+// ------------------------------------------------------------------------------------------
+template <typename T, int MODE, int NROW, int TG, int NRHS, int BLOCK, int MINB, int DEPTH>
+__global__ void __launch_bounds__(BLOCK, MINB) dslash_pair_kernel(const DslashArgs<T, NRHS> a)
+{
+    typedef typename Cplx<T>::type C;
+    static_assert(NRHS % 2 == 0, "the pair kernel splits an even number of vectors");
+    constexpr int NV = NRHS / 2;                     // vectors per lane: r = half + 2 j
+    constexpr int SITES = BLOCK / 2;
+    extern __shared__ __align__(16) unsigned char staged_smem[];
+    C (*ring)[SITES] = reinterpret_cast<C (*)[SITES]>(staged_smem);        // [DEPTH * 3 NROW][SITES]
+    if (a.check_flag) {
+        bool all_done = true;
+#pragma unroll
+        for (int r = 0; r < NRHS; ++r) all_done = all_done && (a.scal[r].flag != 0);
+        if (all_done) return;
+    }
+    const size_t Vh = (size_t)a.L.Vh;
+    const int sl = threadIdx.x >> 1, half = threadIdx.x & 1;
+    // this lane's vectors, picked with static indices (a runtime index into the parameter arrays would spill them)
+    const C *in_[NV], *v_[NV];
+    C *out_[NV];
+#pragma unroll
+    for (int j = 0; j < NV; ++j) {
+        in_[j] = half ? a.in[2 * j + 1] : a.in[2 * j];
+        out_[j] = half ? a.out[2 * j + 1] : a.out[2 * j];
+        v_[j] = half ? a.v[2 * j + 1] : a.v[2 * j];
+    }
+    double dot[NRHS];
+#pragma unroll
+    for (int r = 0; r < NRHS; ++r) dot[r] = 0.0;
+
+#pragma unroll 1
+    for (int chunk = 0; chunk < (MODE == 2 ? a.chunks : 1); ++chunk) {
+        const int tid = (blockIdx.x * (MODE == 2 ? a.chunks : 1) + chunk) * SITES + sl;      // < Vh: Vh % SITES == 0
+        const int cb = traversal_site(a.L, tid);
+        const SiteGeom g = site_geometry(a.L, a.parity, cb);
+        const uint64_t pol_stream = l2_policy_evict_first();
+        const uint64_t pol_keep = l2_policy_evict_last();
+        const C *Uf = a.U + (size_t)(a.parity * 12 * NROW) * Vh + cb;
+        const C *Ub = a.U + (size_t)((1 - a.parity) * 12 * NROW) * Vh;
+
+        // this lane's share of the copies of hop h (an empty group for a unit link)
+        auto issue = [&](int h) {
+            const int mu = h >> 1;
+            const bool fwd = (h & 1) == 0;
+            const bool unit = TG && mu == 3 && (fwd ? g.x3 != 0 : g.x3 != 1);
+            const C *src = fwd ? Uf + (size_t)(mu * 3 * NROW) * Vh : Ub + (size_t)(mu * 3 * NROW) * Vh + g.nb[mu];
+            if (!unit) {
+                // planes 2 i + half, no predicate; with nine planes the last one is split into its real and imaginary half
+#pragma unroll
+                for (int i = 0; i < (3 * NROW) / 2; ++i) {
+                    const int k = 2 * i + half;
+                    cp_async_stream(&ring[(h % DEPTH) * 3 * NROW + k][sl], src + (size_t)k * Vh, pol_stream);
+                }
+                if ((3 * NROW) & 1)
+                    cp_async_stream_half(&ring[(h % DEPTH) * 3 * NROW + 3 * NROW - 1][sl], src + (size_t)(3 * NROW - 1) * Vh, half, pol_stream);
+            }
+            cp_async_commit();
+        };
+#pragma unroll
+        for (int h = 0; h < DEPTH; ++h) issue(h);
+
+        C acc[NV][3];
+#pragma unroll
+        for (int j = 0; j < NV; ++j)
+            acc[j][0].x = acc[j][0].y = acc[j][1].x = acc[j][1].y = acc[j][2].x = acc[j][2].y = (T)0;
+        if (MODE >= 1) {
+#pragma unroll
+            for (int j = 0; j < NV; ++j)
+#pragma unroll
+                for (int c = 0; c < 3; ++c) prefetch_l2(v_[j] + (size_t)c * Vh + cb);
+        }
+
+        auto hop_site = [&](int h) { return (h & 1) == 0 ? g.nf[h >> 1] : g.nb[h >> 1]; };
+        auto hop_sign = [&](int h) { return (T)((h & 1) == 0 ? g.sf[h >> 1] : g.sb[h >> 1]); };
+        C pbuf[2][NV][3];
+#pragma unroll
+        for (int j = 0; j < NV; ++j) load_spinor<T, C>(pbuf[0][j], in_[j], Vh, hop_site(0), hop_sign(0), pol_keep);
+#pragma unroll
+        for (int h = 0; h < 8; ++h) {
+            const int mu = h >> 1;
+            const bool fwd = (h & 1) == 0;
+            const bool unit = TG && mu == 3 && (fwd ? g.x3 != 0 : g.x3 != 1);
+            C (&p)[NV][3] = pbuf[h & 1];
+            if (h + 1 < 8) {
+#pragma unroll
+                for (int j = 0; j < NV; ++j)
+                    load_spinor<T, C>(pbuf[(h + 1) & 1][j], in_[j], Vh, hop_site(h + 1), hop_sign(h + 1), pol_keep);
+            }
+            cp_async_wait((h + DEPTH < 8 ? h + DEPTH : 8) - h - 1);     // this lane's planes of hop h have landed
+            __syncwarp();                                               // ... and so have the partner's
+            if (!unit) {
+                C u[9];
+#pragma unroll
+                for (int k = 0; k < 3 * NROW; ++k) u[k] = ring[(h % DEPTH) * 3 * NROW + k][sl];
+                if (NROW == 2) reconstruct_third_row<C>(u);
+#pragma unroll
+                for (int j = 0; j < NV; ++j) {
+                    if (fwd) mat_vec_acc<T, C>(acc[j], u, p[j]); else matdag_vec_acc<T, C>(acc[j], u, p[j]);
+                }
+            } else {
+#pragma unroll
+                for (int j = 0; j < NV; ++j) vec_acc<C>(acc[j], p[j]);
+            }
+            __syncwarp();                                               // both lanes have read the column before it is refilled
+            if (h + DEPTH < 8) issue(h + DEPTH);
+        }
+
+        // epilogue for this lane's vectors (dslash_epilogue, with r = half + 2 j)
+        if (MODE >= 1) {
+            C vv[NV][3];
+#pragma unroll
+            for (int j = 0; j < NV; ++j)
+#pragma unroll
+                for (int c = 0; c < 3; ++c) vv[j][c] = ld_stream(v_[j] + (size_t)c * Vh + cb, pol_stream);
+#pragma unroll
+            for (int j = 0; j < NV; ++j) {
+#pragma unroll
+                for (int c = 0; c < 3; ++c) {
+                    C o;
+                    o.x = fma(a.m2, vv[j][c].x, -acc[j][c].x);
+                    o.y = fma(a.m2, vv[j][c].y, -acc[j][c].y);
+                    out_[j][(size_t)c * Vh + cb] = o;
+                    // dot[] is indexed statically: lane `half` owns the even or the odd vectors
+                    const double d = (double)vv[j][c].x * (double)o.x + (double)vv[j][c].y * (double)o.y;
+                    if (MODE == 2) { if (half == 0) dot[2 * j] += d; else dot[2 * j + 1] += d; }
+                }
+            }
+        } else {
+#pragma unroll
+            for (int j = 0; j < NV; ++j)
+#pragma unroll
+                for (int c = 0; c < 3; ++c) out_[j][(size_t)c * Vh + cb] = acc[j][c];
+        }
+    }
+    dslash_reduce<T, MODE, NRHS, BLOCK>(a, dot);
+}
+
 } // namespace qcd

@@ -98,9 +98,39 @@ static cudaError_t launch_staged(const DslashLaunch &d)
     return cudaGetLastError();
 }
 
+// Pair kernel (two lanes per site, NRHS / 2 vectors each; dslash.cuh): 128 threads = 64 sites per block.
+enum { PAIR_BLOCK = 128, PAIR_DEPTH = 4 };
+template <typename T, int MODE, int NROW, int TG, int NRHS, int MINB>
+static cudaError_t launch_pair(const DslashLaunch &d)
+{
+    typedef typename Cplx<T>::type C;
+    const size_t smem = (size_t)PAIR_DEPTH * 3 * NROW * (PAIR_BLOCK / 2) * sizeof(C);
+    auto kernel = dslash_pair_kernel<T, MODE, NROW, TG, NRHS, PAIR_BLOCK, MINB, PAIR_DEPTH>;
+    {
+        const cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+    }
+    DslashArgs<T, NRHS> a;
+    a.L = d.L; a.parity = d.parity; a.U = (const C *)d.U;
+    for (int r = 0; r < NRHS; ++r) { a.in[r] = (const C *)d.in[r]; a.out[r] = (C *)d.out[r]; a.v[r] = (const C *)d.v[r]; }
+    a.m2 = (T)d.m2; a.partials = d.partials; a.scal = d.scal; a.check_flag = d.check_flag;
+    const int sites = PAIR_BLOCK / 2;
+    a.chunks = MODE == 2 ? reduce_chunks(d.L.Vh, sites) : 1;
+    while (a.chunks > 1 && (d.L.Vh / sites) % a.chunks) --a.chunks;       // whole chunks only: every lane of the block is active
+    const int grid = d.L.Vh / (sites * a.chunks);
+    kernel<<<grid, PAIR_BLOCK, smem, d.stream>>>(a);
+    return cudaGetLastError();
+}
+
 template <typename T, int MODE, int NROW, int TG, int NRHS>
 static cudaError_t launch_nrhs(const DslashLaunch &d)
 {
+    // variants 6 / 7 force the pair kernel at a 168- / 128-register cap (A/B sweeps); it needs an even number of vectors
+    // and a volume of whole 64-site blocks
+    if constexpr (MODE != 1 && NRHS >= 4 && NRHS % 2 == 0) {
+        if ((d.variant == 6 || d.variant == 7) && d.L.Vh % (PAIR_BLOCK / 2) == 0)
+            return d.variant == 6 ? launch_pair<T, MODE, NROW, TG, NRHS, 3>(d) : launch_pair<T, MODE, NROW, TG, NRHS, 4>(d);
+    }
     // variant 4 forces the staged kernel, variant 5 the register kernel (A/B sweeps); otherwise the
     // staged kernel serves the (precision, NRHS, link rows) where it measured faster at 64^4
     // (profiles/README.md "staged vs register kernel"): fp64 n = 3, 4; fp32 n = 8, and n >= 4 on two-row links

@@ -98,6 +98,21 @@ __device__ __forceinline__ void cp_async_stream(float2 *smem_dst, const float2 *
     const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
     asm volatile("cp.async.ca.shared.global.L2::cache_hint [%0], [%1], 8, %2;" :: "r"(d), "l"(src), "l"(pol) : "memory");
 }
+// one HALF of a complex number (lane `half` of a pair copies the real or the imaginary part): lets two lanes split an
+// odd number of planes without a predicated copy (a predicated cp.async with an L2 policy operand is what ptxas 12.9
+// turns into an instruction sm_100a rejects)
+__device__ __forceinline__ void cp_async_stream_half(double2 *smem_dst, const double2 *src, int half, uint64_t pol)
+{
+    const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst) + 8u * (unsigned)half;
+    const char *s = reinterpret_cast<const char *>(src) + 8 * half;
+    asm volatile("cp.async.ca.shared.global.L2::cache_hint [%0], [%1], 8, %2;" :: "r"(d), "l"(s), "l"(pol) : "memory");
+}
+__device__ __forceinline__ void cp_async_stream_half(float2 *smem_dst, const float2 *src, int half, uint64_t pol)
+{
+    const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst) + 4u * (unsigned)half;
+    const char *s = reinterpret_cast<const char *>(src) + 4 * half;
+    asm volatile("cp.async.ca.shared.global.L2::cache_hint [%0], [%1], 4, %2;" :: "r"(d), "l"(s), "l"(pol) : "memory");
+}
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 // wait until at most `pending` of this thread's most recent groups are still in flight
 // (the operand must be an immediate: the switch folds once the caller's loop is unrolled)

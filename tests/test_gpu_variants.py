@@ -252,7 +252,7 @@ def test_dslash_multi(q, n, prec, kind_name, tg):
         f.buf.zero_()
     refs = ov.dslash_multi(dims, Ur, [_rounded(p, prec) for p in phis], -1)
     first = None
-    for kernel in (0, 4, 5):        # library's choice; staged (links through shared memory); register kernel
+    for kernel in (0, 4, 5, 6, 7):  # library's choice; staged (links through shared memory); register kernel; pair kernel at two register caps
         ctx.qcd_set_dslash_variant(kernel)
         for f in fout:
             f.buf.zero_()
