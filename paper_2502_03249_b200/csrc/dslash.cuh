@@ -126,6 +126,17 @@ __device__ __forceinline__ void load_spinor(C p[3], const C *f, size_t Vh, int s
     for (int c = 0; c < 3; ++c) { p[c].x = flip_sign(p[c].x, neg); p[c].y = flip_sign(p[c].y, neg); }
 }
 
+// the same from the shared-memory tile of a block (dslash_kernel, TILE): colour planes `stride` elements apart
+template <typename T, typename C>
+__device__ __forceinline__ void load_spinor_tile(C p[3], const C *t, int stride, T sign)
+{
+#pragma unroll
+    for (int c = 0; c < 3; ++c) p[c] = t[(size_t)c * stride];
+    const unsigned neg = sign < (T)0 ? 1u : 0u;
+#pragma unroll
+    for (int c = 0; c < 3; ++c) { p[c].x = flip_sign(p[c].x, neg); p[c].y = flip_sign(p[c].y, neg); }
+}
+
 template <typename C>
 __device__ __forceinline__ void vec_acc(C acc[3], const C p[3])
 {
@@ -199,10 +210,17 @@ __device__ __forceinline__ void dslash_reduce(const DslashArgs<T, NRHS> &a, doub
     }
 }
 
-template <typename T, int MODE, int NROW, int TG, int NRHS, int BLOCK, int MINB>
+// TILE (several vectors; the host checks that a block's BLOCK sites are R = BLOCK / h whole x0-rows of one (x2, x3) plane):
+// the x0 and x1 neighbours of a block's sites lie in the R + 2 rows x1 - 1 ... x1 + R of that plane -- 6 rows for the 16 row
+// loads of the four hops at 64^4.  They are copied once into shared memory (cp.async, all vectors, then one barrier) and
+// the hops mu = 0, 1 read them from there: 22 instead of 32 row fetches per vector go through the L2 -> SM path, the one that
+// saturates (~10 TB/s under the power cap) once several vectors share a link.  Same values, same FMA
+// order: bitwise identical results.
+template <typename T, int MODE, int NROW, int TG, int NRHS, int BLOCK, int MINB, bool TILE = false>
 __global__ void __launch_bounds__(BLOCK, MINB) dslash_kernel(const DslashArgs<T, NRHS> a)
 {
     typedef typename Cplx<T>::type C;
+    extern __shared__ __align__(16) unsigned char tile_smem[];
     if (a.check_flag) {
         bool all_done = true;
 #pragma unroll
@@ -224,6 +242,26 @@ __global__ void __launch_bounds__(BLOCK, MINB) dslash_kernel(const DslashArgs<T,
     const int tid = (blockIdx.x * (MODE == 2 ? a.chunks : 1) + chunk) * BLOCK + threadIdx.x;
     const bool active = tid < a.L.Vh;
     const int cb = active ? traversal_site(a.L, tid) : tid;
+    const int tile_w = BLOCK + 2 * a.L.h;                         // elements per (vector, colour) row set: R + 2 rows of h sites
+    C *tile = reinterpret_cast<C *>(tile_smem);                   // [NRHS * 3][tile_w]
+    if (TILE) {
+        // every thread of the block is active (Vh % BLOCK == 0) and cb = cb0 + threadIdx.x
+        if (chunk > 0) __syncthreads();                           // the previous chunk's tile has been read by everyone
+        const int cb0 = cb - (int)threadIdx.x;
+        const int x1_0 = (int)(((unsigned)cb0 / (unsigned)a.L.h) % (unsigned)a.L.N1);
+        const int plane0 = cb0 - x1_0 * a.L.h;
+        for (int e = threadIdx.x; e < tile_w; e += BLOCK) {
+            const int row = e / a.L.h, xh = e - row * a.L.h;
+            int x1s = x1_0 - 1 + row;
+            x1s += x1s < 0 ? a.L.N1 : (x1s >= a.L.N1 ? -a.L.N1 : 0);
+            const size_t src = (size_t)(plane0 + x1s * a.L.h + xh);
+#pragma unroll
+            for (int r = 0; r < NRHS; ++r)
+#pragma unroll
+                for (int c = 0; c < 3; ++c) cp_async_plain(&tile[(size_t)(r * 3 + c) * tile_w + e], a.in[r] + (size_t)c * Vh + src);
+        }
+        cp_async_commit();
+    }
     if (active) {
         const SiteGeom g = site_geometry(a.L, a.parity, cb);
         const uint64_t pol_stream = l2_policy_evict_first();
@@ -243,6 +281,11 @@ __global__ void __launch_bounds__(BLOCK, MINB) dslash_kernel(const DslashArgs<T,
 #pragma unroll
                 for (int c = 0; c < 3; ++c) prefetch_l2(a.v[r] + (size_t)c * Vh + cb);
         }
+
+        if (TILE) { cp_async_wait(0); __syncthreads(); }
+        // element of the tile that holds site cb itself (row rho + 1 of the R + 2 rows): the x0 neighbours sit in the same row,
+        // the x1 neighbours one row up / down
+        const int tile_c = a.L.h + (int)threadIdx.x;
 
 #pragma unroll
         for (int mu = 0; mu < 4; ++mu) {
@@ -302,8 +345,14 @@ __global__ void __launch_bounds__(BLOCK, MINB) dslash_kernel(const DslashArgs<T,
                 {
                     C u[9], p[NRHS][3];
                     if (!unit_f) load_link<NROW, C>(u, ufp, Vh, pol_stream);
+                    if (TILE && mu < 2) {
+                        const int e = mu == 0 ? tile_c + (g.nf[0] - cb) : tile_c + a.L.h;
 #pragma unroll
-                    for (int r = 0; r < NRHS; ++r) load_spinor<T, C>(p[r], a.in[r], Vh, g.nf[mu], sf, pol_keep);
+                        for (int r = 0; r < NRHS; ++r) load_spinor_tile<T, C>(p[r], tile + (size_t)(r * 3) * tile_w + e, tile_w, sf);
+                    } else {
+#pragma unroll
+                        for (int r = 0; r < NRHS; ++r) load_spinor<T, C>(p[r], a.in[r], Vh, g.nf[mu], sf, pol_keep);
+                    }
                     if (!unit_f) {
                         if (NROW == 2) reconstruct_third_row<C>(u);
 #pragma unroll
@@ -316,8 +365,14 @@ __global__ void __launch_bounds__(BLOCK, MINB) dslash_kernel(const DslashArgs<T,
                 {
                     C u[9], p[NRHS][3];
                     if (!unit_b) load_link<NROW, C>(u, ubp, Vh, pol_stream);
+                    if (TILE && mu < 2) {
+                        const int e = mu == 0 ? tile_c + (g.nb[0] - cb) : tile_c - a.L.h;
 #pragma unroll
-                    for (int r = 0; r < NRHS; ++r) load_spinor<T, C>(p[r], a.in[r], Vh, g.nb[mu], sb, pol_keep);
+                        for (int r = 0; r < NRHS; ++r) load_spinor_tile<T, C>(p[r], tile + (size_t)(r * 3) * tile_w + e, tile_w, sb);
+                    } else {
+#pragma unroll
+                        for (int r = 0; r < NRHS; ++r) load_spinor<T, C>(p[r], a.in[r], Vh, g.nb[mu], sb, pol_keep);
+                    }
                     if (!unit_b) {
                         if (NROW == 2) reconstruct_third_row<C>(u);
 #pragma unroll
@@ -593,6 +648,129 @@ __global__ void __launch_bounds__(BLOCK, MINB) dslash_pair_kernel(const DslashAr
 #pragma unroll
                 for (int c = 0; c < 3; ++c) out_[j][(size_t)c * Vh + cb] = acc[j][c];
         }
+    }
+    dslash_reduce<T, MODE, NRHS, BLOCK>(a, dot);
+}
+
+// ------------------------------------------------------------------------------------------
+// Rolled variant for many vectors (NRHS >= 5).  ncu on the fully unrolled kernels at n = 8 (profiles/README.md, r02):
+// 4200 SASS instructions = 68 KB of straight-line code per thread, `gcc__cache_requests_type_instruction` at 78-87 % of
+// its peak, every memory unit below 65 %, fp64 pipe at 33-40 % -- and four structurally different kernels (register,
+// staged, pair, shared-memory tile) within 3 % of one another.  Eight warps per SM walking 68 KB of code at different
+// places miss the 32 KB instruction cache on every line: the kernels are bound by INSTRUCTION FETCH.  Here the loop over
+// the four directions is NOT unrolled (the body -- a forward and a backward hop for all vectors -- is a quarter of the
+// code, and the neighbour index, phase and seam sign of direction mu are computed arithmetically from mu instead of being
+// read from eight-entry arrays).  Per vector the FMAs and their order are those of the other kernels: bitwise identical.
+// ------------------------------------------------------------------------------------------
+template <typename T, typename C>
+__device__ __forceinline__ void load_spinor_neg(C p[3], const C *f, size_t Vh, int site, unsigned neg, uint64_t pol)
+{
+#pragma unroll
+    for (int c = 0; c < 3; ++c) p[c] = ld_keep(f + (size_t)c * Vh + site, pol);
+#pragma unroll
+    for (int c = 0; c < 3; ++c) { p[c].x = flip_sign(p[c].x, neg); p[c].y = flip_sign(p[c].y, neg); }
+}
+
+template <typename T, int MODE, int NROW, int TG, int NRHS, int BLOCK, int MINB>
+__global__ void __launch_bounds__(BLOCK, MINB) dslash_rolled_kernel(const DslashArgs<T, NRHS> a)
+{
+    typedef typename Cplx<T>::type C;
+    if (a.check_flag) {
+        bool all_done = true;
+#pragma unroll
+        for (int r = 0; r < NRHS; ++r) all_done = all_done && (a.scal[r].flag != 0);
+        if (all_done) return;
+    }
+    const size_t Vh = (size_t)a.L.Vh;
+    double dot[NRHS];
+#pragma unroll
+    for (int r = 0; r < NRHS; ++r) dot[r] = 0.0;
+
+#pragma unroll 1
+    for (int chunk = 0; chunk < (MODE == 2 ? a.chunks : 1); ++chunk) {
+    const int tid = (blockIdx.x * (MODE == 2 ? a.chunks : 1) + chunk) * BLOCK + threadIdx.x;
+    const bool active = tid < a.L.Vh;
+    const int cb = active ? traversal_site(a.L, tid) : tid;
+    if (active) {
+        // coordinates of the site (lattice.cuh site_geometry, here kept as coordinates: the per-direction quantities are
+        // formed inside the rolled loop)
+        const unsigned ucb = (unsigned)cb;
+        const int xh = (int)(ucb % (unsigned)a.L.h);
+        unsigned q = ucb / (unsigned)a.L.h;
+        const int x1 = (int)(q % (unsigned)a.L.N1);
+        q /= (unsigned)a.L.N1;
+        const int x2 = (int)(q % (unsigned)a.L.N2);
+        const int x3 = (int)(q / (unsigned)a.L.N2);
+        const int rp = (x1 + x2 + x3 + a.parity) & 1;
+        const uint64_t pol_stream = l2_policy_evict_first();
+        const uint64_t pol_keep = l2_policy_evict_last();
+        const C *uf = a.U + (size_t)(a.parity * 12 * NROW) * Vh + cb;          // U_{x,mu}, advanced by one link per direction
+        const C *ub = a.U + (size_t)((1 - a.parity) * 12 * NROW) * Vh;         // U_{x-mu,mu}
+
+        C acc[NRHS][3];
+#pragma unroll
+        for (int r = 0; r < NRHS; ++r)
+            acc[r][0].x = acc[r][0].y = acc[r][1].x = acc[r][1].y = acc[r][2].x = acc[r][2].y = (T)0;
+        if (MODE >= 1) {
+#pragma unroll
+            for (int r = 0; r < NRHS; ++r)
+#pragma unroll
+                for (int c = 0; c < 3; ++c) prefetch_l2(a.v[r] + (size_t)c * Vh + cb);
+        }
+
+        int xm = 0, Nm = 0, sm = 1;           // coordinate, extent and cb stride of direction mu (mu = 0 is special-cased)
+        unsigned e = 0;                       // eta_mu(x) = (-1)^e,  e = x0 + ... + x_{mu-1} mod 2
+#pragma unroll 1
+        for (int mu = 0; mu < 4; ++mu) {
+            int nf, nb;
+            if (mu == 0) {
+                nf = rp ? ((xh + 1 == a.L.h) ? cb - (a.L.h - 1) : cb + 1) : cb;
+                nb = rp ? cb : ((xh == 0) ? cb + (a.L.h - 1) : cb - 1);
+            } else {
+                xm = mu == 1 ? x1 : (mu == 2 ? x2 : x3);
+                Nm = mu == 1 ? a.L.N1 : (mu == 2 ? a.L.N2 : a.L.N3);
+                sm = mu == 1 ? a.L.s1 : (mu == 2 ? a.L.s2 : a.L.s3);
+                nf = (xm + 1 == Nm) ? cb - (Nm - 1) * sm : cb + sm;
+                nb = (xm == 0) ? cb + (Nm - 1) * sm : cb - sm;
+                e = (unsigned)(rp + (mu >= 2 ? x1 : 0) + (mu >= 3 ? x2 : 0)) & 1u;
+            }
+            const unsigned negf = e ^ ((mu == 3 && x3 + 1 == a.L.N3) ? 1u : 0u);      // eta, times -1 across the time seam
+            const unsigned negb = (e ^ 1u) ^ ((mu == 3 && x3 == 0) ? 1u : 0u);        // MINUS eta, times -1 across the seam
+            const bool unit_f = TG && mu == 3 && x3 != 0;
+            const bool unit_b = TG && mu == 3 && x3 != 1;
+            {
+                C u[9], p[NRHS][3];
+                if (!unit_f) load_link<NROW, C>(u, uf, Vh, pol_stream);
+#pragma unroll
+                for (int r = 0; r < NRHS; ++r) load_spinor_neg<T, C>(p[r], a.in[r], Vh, nf, negf, pol_keep);
+                if (!unit_f) {
+                    if (NROW == 2) reconstruct_third_row<C>(u);
+#pragma unroll
+                    for (int r = 0; r < NRHS; ++r) mat_vec_acc<T, C>(acc[r], u, p[r]);
+                } else {
+#pragma unroll
+                    for (int r = 0; r < NRHS; ++r) vec_acc<C>(acc[r], p[r]);
+                }
+            }
+            {
+                C u[9], p[NRHS][3];
+                if (!unit_b) load_link<NROW, C>(u, ub + nb, Vh, pol_stream);
+#pragma unroll
+                for (int r = 0; r < NRHS; ++r) load_spinor_neg<T, C>(p[r], a.in[r], Vh, nb, negb, pol_keep);
+                if (!unit_b) {
+                    if (NROW == 2) reconstruct_third_row<C>(u);
+#pragma unroll
+                    for (int r = 0; r < NRHS; ++r) matdag_vec_acc<T, C>(acc[r], u, p[r]);
+                } else {
+#pragma unroll
+                    for (int r = 0; r < NRHS; ++r) vec_acc<C>(acc[r], p[r]);
+                }
+            }
+            uf += (size_t)(3 * NROW) * Vh;
+            ub += (size_t)(3 * NROW) * Vh;
+        }
+        dslash_epilogue<T, MODE, NRHS>(a, cb, acc, dot, pol_stream);
+    }
     }
     dslash_reduce<T, MODE, NRHS, BLOCK>(a, dot);
 }

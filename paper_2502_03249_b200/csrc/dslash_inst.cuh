@@ -70,6 +70,51 @@ static cudaError_t launch_cfg(const DslashLaunch &d)
     return cudaGetLastError();
 }
 
+// Register kernel with the x0 / x1 neighbour rows of a block in shared memory (dslash.cuh, TILE).  Needs a block to be whole
+// x0-rows of one (x2, x3) plane: BLOCK % h == 0, N1 % (BLOCK / h) == 0 (then Vh % BLOCK == 0 and the traversal chunks, whole
+// x2-rows, keep a block's sites consecutive).
+static inline bool tile_eligible(const Lattice &L, int block)
+{
+    return L.h <= block && block % L.h == 0 && L.N1 % (block / L.h) == 0;
+}
+template <typename T, int MODE, int NROW, int TG, int NRHS>
+static cudaError_t launch_tile(const DslashLaunch &d)
+{
+    typedef typename Cplx<T>::type C;
+    enum { BLOCK = DslashCfg<T, NRHS>::BLOCK, MINB = DslashCfg<T, NRHS>::MINB };
+    const size_t smem = (size_t)NRHS * 3 * (BLOCK + 2 * d.L.h) * sizeof(C);
+    auto kernel = dslash_kernel<T, MODE, NROW, TG, NRHS, BLOCK, MINB, true>;
+    {
+        const cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+    }
+    DslashArgs<T, NRHS> a;
+    a.L = d.L; a.parity = d.parity; a.U = (const C *)d.U;
+    for (int r = 0; r < NRHS; ++r) { a.in[r] = (const C *)d.in[r]; a.out[r] = (C *)d.out[r]; a.v[r] = (const C *)d.v[r]; }
+    a.m2 = (T)d.m2; a.partials = d.partials; a.scal = d.scal; a.check_flag = d.check_flag;
+    a.chunks = MODE == 2 ? reduce_chunks(d.L.Vh, BLOCK) : 1;
+    while (a.chunks > 1 && (d.L.Vh / BLOCK) % a.chunks) --a.chunks;
+    const int grid = d.L.Vh / (BLOCK * a.chunks);
+    kernel<<<grid, BLOCK, smem, d.stream>>>(a);
+    return cudaGetLastError();
+}
+
+template <typename T, int MODE, int NROW, int TG, int NRHS>
+static cudaError_t launch_rolled(const DslashLaunch &d)
+{
+    typedef typename Cplx<T>::type C;
+    enum { BLOCK = DslashCfg<T, NRHS>::BLOCK, MINB = DslashCfg<T, NRHS>::MINB };
+    DslashArgs<T, NRHS> a;
+    a.L = d.L; a.parity = d.parity; a.U = (const C *)d.U;
+    for (int r = 0; r < NRHS; ++r) { a.in[r] = (const C *)d.in[r]; a.out[r] = (C *)d.out[r]; a.v[r] = (const C *)d.v[r]; }
+    a.m2 = (T)d.m2; a.partials = d.partials; a.scal = d.scal; a.check_flag = d.check_flag;
+    a.chunks = MODE == 2 ? reduce_chunks(d.L.Vh, BLOCK) : 1;
+    const int per_block = BLOCK * a.chunks;
+    const int grid = (d.L.Vh + per_block - 1) / per_block;
+    dslash_rolled_kernel<T, MODE, NROW, TG, NRHS, BLOCK, MINB><<<grid, BLOCK, 0, d.stream>>>(a);
+    return cudaGetLastError();
+}
+
 // Staged kernel (links through shared memory by cp.async, dslash.cuh): ring of STAGE_DEPTH hops.
 enum { STAGE_DEPTH = 4 };
 template <typename T, int NRHS> struct StagedCfg { enum { BLOCK = 128, MINB = sizeof(T) == 8 ? (NRHS <= 4 ? 3 : 2) : (NRHS <= 4 ? 4 : 3) }; };
@@ -127,6 +172,16 @@ static cudaError_t launch_nrhs(const DslashLaunch &d)
 {
     // variants 6 / 7 force the pair kernel at a 168- / 128-register cap (A/B sweeps); it needs an even number of vectors
     // and a volume of whole 64-site blocks
+    // variant 9 forces the rolled kernel (direction loop not unrolled: a quarter of the code; dslash.cuh)
+    if constexpr (MODE != 1 && NRHS >= 3) {
+        if (d.variant == 9) return launch_rolled<T, MODE, NROW, TG, NRHS>(d);
+    }
+    // variant 8 forces the register kernel with the shared-memory tile of the x0 / x1 neighbour rows
+    if constexpr (MODE != 1 && (NRHS == 4 || NRHS == 8)) {
+        if (d.variant == 8 && tile_eligible(d.L, DslashCfg<T, NRHS>::BLOCK) &&
+            (size_t)NRHS * 3 * (DslashCfg<T, NRHS>::BLOCK + 2 * d.L.h) * sizeof(typename Cplx<T>::type) <= 200 * 1024)
+            return launch_tile<T, MODE, NROW, TG, NRHS>(d);
+    }
     if constexpr (MODE != 1 && NRHS >= 4 && NRHS % 2 == 0) {
         if ((d.variant == 6 || d.variant == 7) && d.L.Vh % (PAIR_BLOCK / 2) == 0)
             return d.variant == 6 ? launch_pair<T, MODE, NROW, TG, NRHS, 3>(d) : launch_pair<T, MODE, NROW, TG, NRHS, 4>(d);

@@ -113,6 +113,17 @@ __device__ __forceinline__ void cp_async_stream_half(float2 *smem_dst, const flo
     const char *s = reinterpret_cast<const char *>(src) + 4 * half;
     asm volatile("cp.async.ca.shared.global.L2::cache_hint [%0], [%1], 4, %2;" :: "r"(d), "l"(s), "l"(pol) : "memory");
 }
+// the same copies without an L2 policy operand (used where the copy is predicated, see cp_async_stream_half)
+__device__ __forceinline__ void cp_async_plain(double2 *smem_dst, const double2 *src)
+{
+    const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" :: "r"(d), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async_plain(float2 *smem_dst, const float2 *src)
+{
+    const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" :: "r"(d), "l"(src) : "memory");
+}
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 // wait until at most `pending` of this thread's most recent groups are still in flight
 // (the operand must be an immediate: the switch folds once the caller's loop is unrolled)

@@ -418,7 +418,7 @@ extern "C" qcd_status qcd_cg_timeline_read(qcd_ctx *ctx, unsigned long long *hos
 extern "C" qcd_status qcd_set_dslash_variant(qcd_ctx *ctx, int variant)
 {
     if (!ctx) return QCD_EINVAL;
-    if (variant < 0 || variant > 7) return fail(ctx, QCD_EINVAL, "qcd_set_dslash_variant: unknown variant");
+    if (variant < 0 || variant > 9) return fail(ctx, QCD_EINVAL, "qcd_set_dslash_variant: unknown variant");
     ctx->variant = variant;
     return QCD_OK;
 }

@@ -252,7 +252,7 @@ def test_dslash_multi(q, n, prec, kind_name, tg):
         f.buf.zero_()
     refs = ov.dslash_multi(dims, Ur, [_rounded(p, prec) for p in phis], -1)
     first = None
-    for kernel in (0, 4, 5, 6, 7):  # library's choice; staged (links through shared memory); register kernel; pair kernel at two register caps
+    for kernel in (0, 4, 5, 6, 7, 8, 9):  # library's choice; staged (links through shared memory); register kernel; pair kernel at two register caps; register kernel with the x0-x1 tile; rolled direction loop
         ctx.qcd_set_dslash_variant(kernel)
         for f in fout:
             f.buf.zero_()
@@ -267,6 +267,58 @@ def test_dslash_multi(q, n, prec, kind_name, tg):
         else:                        # same FMAs in the same order per site, whichever way the operands arrive
             assert all(np.array_equal(a, b) for a, b in zip(first, got)), kernel
     ctx.close()
+
+
+@pytest.mark.parametrize("prec", [64, 32])
+@pytest.mark.parametrize("dims,chunk", [((32, 8, 2, 4), 0), ((16, 16, 4, 2), 1), ((16, 16, 4, 2), 2), ((64, 4, 2, 2), 0)])
+def test_dslash_tile_and_pair_kernels_on_row_aligned_lattices(q, dims, chunk, prec):
+    """The register kernel with the x0 / x1 neighbour rows of a block in shared memory (variant 8) needs a block of 128
+    sites to be whole x0-rows of one (x2, x3) plane; (8,4,6,10) of test_dslash_multi is not such a lattice and runs the
+    library's choice there.  Here it does run: rows of 16, 8 and 32 sites, x1 and x2 wraps inside a block's neighbourhood,
+    with and without traversal chunking, plain Dslash (MODE 0) and, through the lock-step CG, the reducing kernel (MODE 2).
+    Bitwise equal to the library's choice, and equal to the oracle within tolerance."""
+    U = qcd_inputs.gauge_field(dims, "haar", seed=0)
+    par = qcd_inputs.site_parity(dims)
+    for n in (4, 8):
+        ctx = q.Context(dims, prec, nrhs=n)
+        ctx.qcd_set_traversal_chunk(chunk)
+        fU = ctx.field(q.QCD_GAUGE).upload(U)
+        phis = [qcd_inputs.gaussian_spinor(dims, seed=30 + i) for i in range(n)]
+        fin = [ctx.field(q.QCD_SPINOR_FULL).upload(p) for p in phis]
+        fout = [ctx.field(q.QCD_SPINOR_FULL) for _ in range(n)]
+        refs = ov.dslash_multi(dims, _rounded(U, prec), [_rounded(p, prec) for p in phis], -1)
+        first = None
+        for kernel in (0, 8, 6, 5, 9):
+            ctx.qcd_set_dslash_variant(kernel)
+            for f in fout:
+                f.buf.fill_(255)
+            ctx.qcd_dslash_eo_multi(fU, fout, fin)
+            ctx.qcd_dslash_oe_multi(fU, fout, fin)
+            got = [f.download() for f in fout]
+            for i in range(n):
+                for p in (0, 1):
+                    assert dslash_rel_err(got[i][par == p], refs[i][par == p]) <= DSLASH_TOL[prec], (n, kernel, i, p)
+            if first is None:
+                first = got
+            else:
+                assert all(np.array_equal(a, b) for a, b in zip(first, got)), (n, kernel)
+        # MODE 2 through the lock-step CG: same iteration counts and solutions whichever kernel applies M
+        m, tol = 0.3, (1e-10 if prec == 64 else 1e-5)
+        srcs = [qcd_inputs.gaussian_source(dims, seed=40 + i) for i in range(n)]
+        fb = [ctx.field(q.QCD_SPINOR_EVEN).upload(s_) for s_ in srcs]
+        fx = [ctx.field(q.QCD_SPINOR_EVEN) for _ in range(n)]
+        sols = {}
+        for kernel in (0, 8):
+            ctx.qcd_set_dslash_variant(kernel)
+            infos = ctx.qcd_cg_solve_multi(fU, fb, fx, m, tol, 5000)
+            assert all(i["converged"] for i in infos)
+            sols[kernel] = ([i["iters"] for i in infos], [f.download() for f in fx])
+        assert sols[0][0] == sols[8][0]
+        for a, b in zip(sols[0][1], sols[8][1]):
+            assert np.allclose(a, b, rtol=0, atol=(1e-12 if prec == 64 else 1e-5) * np.abs(a).max())
+        _, oinfo = oracle.cg(dims, _rounded(U, prec).astype(ctx.cdtype), _rounded(srcs[0], prec).astype(ctx.cdtype), m, tol, 5000)
+        assert iters_close(sols[8][0][0], oinfo["iters"])
+        ctx.close()
 
 
 @pytest.mark.parametrize("prec,n", [(64, 2), (64, 3), (64, 8), (32, 4)])
