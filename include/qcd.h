@@ -263,6 +263,10 @@ qcd_status qcd_stream_read_resident(qcd_ctx *ctx, const qcd_field *f, int passes
  *   6, 7 : force the pair kernel (two adjacent lanes per site, half of the vectors each, the link shared through the
  *       cp.async ring) under a 168- / 128-register cap; applies to an even number of vectors >= 4 on a volume of whole
  *       64-site blocks, otherwise the library's choice runs
+ *   8 : force the register kernel with the x0 / x1 neighbour rows of a block staged in shared memory; applies to 4 or 8
+ *       vectors on lattices where 128 consecutive sites are whole x0-rows of one (x2, x3) plane, otherwise the library's choice
+ *   9 : force the kernel whose loop over the four directions is not unrolled (3 .. 8 vectors)
+ * 6 .. 9 are the round-2 experiments (profiles/README.md); none measured faster than the library's choice.
  * Every variant computes the same result (bitwise).  Unknown variants -> QCD_EINVAL.
  */
 qcd_status qcd_set_dslash_variant(qcd_ctx *ctx, int variant);

@@ -970,14 +970,18 @@ static qcd_status cg_persistent_launch(qcd_ctx *c, bool probe_only, bool *ok)
     CU(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, PERSIST_BLOCK, 0));
     *ok = coop && per_sm > 0;
     if (probe_only || !*ok) return QCD_OK;
-    // at most what is co-resident; when the sites need several passes the grid is shrunk so that the passes are equally full
+    // Every block owns an equally long range of sites (cg_persistent.cuh): launch k blocks on EVERY SM, k the smallest number
+    // of co-resident blocks that covers the sites in one pass (16^4 fp64: 2 x 148 blocks of 112 sites), capped by what is
+    // co-resident (then a block walks its range in several trips); tiny lattices get one block per warp of work.
     int max_grid = per_sm * sms;
     if (max_grid * MAXRHS > c->partials_cap) max_grid = c->partials_cap / MAXRHS;
-    const int quads_per_block = PERSIST_BLOCK / SPLIT;
-    const int passes = (c->L.Vh + max_grid * quads_per_block - 1) / (max_grid * quads_per_block);
-    const int per_pass = (c->L.Vh + passes - 1) / passes;
-    int grid = (per_pass + quads_per_block - 1) / quads_per_block;
+    int k = (wanted_threads + sms * PERSIST_BLOCK - 1) / (sms * PERSIST_BLOCK);
+    if (k > per_sm) k = per_sm;
+    int grid = sms * k;
+    const int by_work = (wanted_threads + 31) / 32;
+    if (grid > by_work) grid = by_work;
     if (grid > max_grid) grid = max_grid;
+    if (grid < 1) grid = 1;
     if (c->timeline_on) CU(c, cudaMemsetAsync(c->d_timeline, 0, 2 * TIMELINE_ITERS * TIMELINE_STAMPS * sizeof(unsigned long long), c->stream));
     void *params[] = { &a };
     LaunchScope ls(c, QCD_K_MISC);
