@@ -289,6 +289,31 @@ def update_routine_report(q, torch, device, peak, dims=(48, 48, 48, 48), iters=5
                                  "source": "PAPER.md:56-62 (other hardware; context only)"}}
 
 
+def config2_sweep_report(q, torch, device, peak, hbm_stream_gbs):
+    """BASELINE.json configs[2]: "Dslash throughput sweep" at 32^4 in both precisions -- the block shapes of the one-vector
+    kernel that qcd_set_dslash_variant exposes (0: 128 threads x 4 resident blocks, the library's choice; 1: 64 x 8;
+    2: 256 x 2; 3: 128 x 3), D_oe launches replayed from a CUDA graph."""
+    import qcd_inputs
+    cfg, U, b = qcd_inputs.config_inputs(2)
+    dims = cfg["dims"]
+    Vh = int(np.prod(dims)) // 2
+    names = {0: "128 threads x 4 blocks/SM (library's choice)", 1: "64 x 8", 2: "256 x 2", 3: "128 x 3"}
+    rows = []
+    for prec in (64, 32):
+        stream = torch.cuda.Stream(device=device)
+        with torch.cuda.stream(stream):
+            ctx = q.Context(dims, prec, device=device, stream=stream)
+            fU = ctx.field(q.QCD_GAUGE).upload(U)
+            fb = ctx.field(q.QCD_SPINOR_EVEN).upload(b)
+            fo = ctx.field(q.QCD_SPINOR_ODD)
+            for v in (0, 1, 2, 3):
+                ctx.qcd_set_dslash_variant(v)
+                ms = min(time_dslash_graph(torch, ctx, stream, fU, fb, fo) for _ in range(2))
+                rows.append(dict(dslash_report(ms, Vh, prec // 8, peak, hbm_stream_gbs), prec=prec, block_shape=names[v]))
+            ctx.close()
+    return {"lattice": list(dims), "rows": rows}
+
+
 # ---- oracle timings ----------------------------------------------------------------------------
 def oracle_dslash_times(oracle, dims, U, b):
     """One oracle D_oe: best of 3 on all host threads, and one run on a single thread."""
@@ -582,6 +607,7 @@ def run_all(args, q, torch, ctx, out, side, cfg, dims, U, b, hb, hx, fU, fb, fx,
                 c.close()
             return t2
         section(side, "variants_table2_32x32x32x32", do_table2)
+        section(side, "config2_dslash_block_shape_sweep", lambda: config2_sweep_report(q, torch, ctx.device, peak, stream_gbs))
         section(side, "cg_small_lattice", lambda: small_lattice_report(q, torch, ctx.device))
         section(side, "cg_update_routine_48x48x48x48", lambda: update_routine_report(q, torch, ctx.device, peak))
         section(side, "size_sweep_fig3", lambda: size_sweep_report(q, torch, ctx.device))
