@@ -127,15 +127,29 @@ def variants_sweep(q, torch, ctx, fU_full, dims, peak, nmulti=(1, 2, 3, 4, 6, 8)
         real = torch.float64 if ctx.precision == 64 else torch.float32
         f.buf.view(real).copy_(torch.randn(f.buf.numel() // rsize, generator=g, device=ctx.device, dtype=real))
     rows = []
+    # the streaming ceiling of the same mix of read and write streams with stencil and arithmetic taken out (qcd_stream_mix):
+    # link planes + 3 n vector planes read, 3 n planes written, every thread at its own index
+    fmix = ctx.field(q.QCD_GAUGE)
+    mix_cache = {}
+
+    def mix_ceiling(read_planes, write_planes):
+        key = (min(read_planes, 72), write_planes)          # the source field has 72 planes; GB/s is intensive
+        if key not in mix_cache:
+            ctx.qcd_stream_mix(fU_full, fmix, key[0], key[1], 2)
+            mix_cache[key] = (key[0] + key[1]) * (fU_full.nbytes // 72) / ctx.qcd_stream_mix(fU_full, fmix, key[0], key[1], 5) / 1e6
+        return mix_cache[key]
+
     for name, fU, nrow, tg in (("full18", fU_full, 3, 0), ("tworow12", f12, 2, 0), ("tworow12+temporal_gauge", f12, 2, 1)):
         ctx.qcd_gauge_set_temporal_unit(fU, bool(tg))
         for n in nmulti:
             ms = time_dslash_multi(torch, ctx, fU, fins[:n], fouts[:n], reps)
             comp, nom = variant_reals(nrow, tg, n, dims[3])
             gbs = comp * rsize * Vh / ms / 1e6
+            ceil_gbs = mix_ceiling((6 if tg else 8) * 3 * nrow + 3 * n, 3 * n)
             rows.append({"links": name, "nmulti": n, "ms": round(ms, 5),
                          "tflops": round(FLOP_PER_SITE * n * Vh / ms / 1e9, 3),
                          "gbs_compulsory": round(gbs, 1), "frac_of_measured_copy_peak": round(gbs / peak, 4),
+                         "stream_mix_ceiling_gbs": round(ceil_gbs, 1), "frac_of_stream_mix_ceiling": round(gbs / ceil_gbs, 4),
                          "ai_nominal_flop_per_byte": round(FLOP_PER_SITE * n / (nom * rsize), 3),
                          # Eq. (2) of the paper: attainable = min(peak, AI x bandwidth); the
                          # bandwidth term binds at every n here.  With the paper's NOMINAL bytes (no cache reuse
@@ -144,7 +158,7 @@ def variants_sweep(q, torch, ctx, fU_full, dims, peak, nmulti=(1, 2, 3, 4, 6, 8)
                          "eq2_attainable_tflops_nominal_ai": round(FLOP_PER_SITE * n / (nom * rsize) * peak / 1e3, 3),
                          "eq2_attainable_tflops_compulsory_ai": round(FLOP_PER_SITE * n / (comp * rsize) * peak / 1e3, 3)})
         ctx.qcd_gauge_set_temporal_unit(fU, False)
-    for f in fins + fouts + [f12]:
+    for f in fins + fouts + [f12, fmix]:
         f.free()
     return rows
 

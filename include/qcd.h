@@ -251,6 +251,16 @@ qcd_status qcd_stream_read(qcd_ctx *ctx, const qcd_field *f, int reps, double *m
  * *ms_per_pass = launch time / passes.  L1 is bypassed, every pass is L2 traffic.  Errors as qcd_stream_read.
  */
 qcd_status qcd_stream_read_resident(qcd_ctx *ctx, const qcd_field *f, int passes, double *ms_per_pass);
+/*
+ * Streaming ceiling of a MIX of read and write streams (measurement hook, the NMULTI kernels): one pass reads 16
+ * bytes per thread from each of the first `read_planes` planes (of Vh complex numbers of the context's precision) of src and writes
+ * 16 bytes to each of the first `write_planes` planes of dst, every thread at its own index -- the DRAM access pattern of a
+ * multi-vector half-Dslash (links + n vectors read once, n vectors written) without stencil, neighbour reads or arithmetic.
+ * `reps` passes, CUDA events on the context stream, synchronises; *ms_per_pass is the average.  GB/s = (read_planes +
+ * write_planes) * Vh * 2 * sizeof(real) / ms.  dst is OVERWRITTEN.  Errors: QCD_EINVAL (NULL, foreign or overlapping fields, more
+ * planes than a field holds, reps < 1), QCD_ECUDA.
+ */
+qcd_status qcd_stream_mix(qcd_ctx *ctx, const qcd_field *src, qcd_field *dst, int read_planes, int write_planes, int reps, double *ms_per_pass);
 
 /*
  * Tuning knob for the Dslash kernels (bench sweeps and A/B tests, Sec. 10):

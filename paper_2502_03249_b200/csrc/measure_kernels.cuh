@@ -52,4 +52,27 @@ __global__ void __launch_bounds__(STREAM_BLOCK) stream_read_resident_kernel(cons
     if (x == 0xfff7a5a5deadbeefULL) *sink = make_double2(0.0, 0.0);
 }
 
+// Streaming ceiling for a MIX of read and write streams (measurement hook): every thread reads 16 bytes from each of
+// `nread` planes of Vh elements and writes 16 bytes to each of `nwrite` planes, all at its own index -- the DRAM access
+// pattern of a multi-vector half-Dslash (links + n input vectors read once, n output vectors written) with the stencil,
+// the neighbour reads and the arithmetic taken out.  What it answers: is the 4.6 TB/s that the n = 8 kernels move the
+// memory system's rate for 26 % writes over ~100 concurrent streams, or the kernels' own limit?
+enum { MIX_BLOCK = 128, MIX_BATCH = 8 };
+__global__ void __launch_bounds__(MIX_BLOCK) stream_mix_kernel(const double2 *__restrict__ src, double2 *__restrict__ dst,
+                                                               size_t plane, int nread, int nwrite)
+{
+    const size_t i = (size_t)blockIdx.x * MIX_BLOCK + threadIdx.x;
+    if (i >= plane) return;
+    const uint64_t pol = l2_policy_evict_first();
+    double2 acc = make_double2(0.0, 0.0);
+    for (int k0 = 0; k0 < nread; k0 += MIX_BATCH) {
+        double2 v[MIX_BATCH];
+#pragma unroll
+        for (int j = 0; j < MIX_BATCH; ++j) v[j] = k0 + j < nread ? ld_stream(src + (size_t)(k0 + j) * plane + i, pol) : make_double2(0.0, 0.0);
+#pragma unroll
+        for (int j = 0; j < MIX_BATCH; ++j) { acc.x += v[j].x; acc.y += v[j].y; }
+    }
+    for (int k = 0; k < nwrite; ++k) dst[(size_t)k * plane + i] = acc;
+}
+
 } // namespace qcd

@@ -712,6 +712,42 @@ extern "C" qcd_status qcd_stream_read_resident(qcd_ctx *ctx, const qcd_field *f,
     return QCD_OK;
 }
 
+// Streaming ceiling of a mix of read and write streams (measure_kernels.cuh).
+extern "C" qcd_status qcd_stream_mix(qcd_ctx *ctx, const qcd_field *src, qcd_field *dst, int read_planes, int write_planes,
+                                     int reps, double *ms_per_pass)
+{
+    if (!ctx) return QCD_EINVAL;
+    if (!src || !dst || src->ctx != ctx || dst->ctx != ctx || reps < 1 || !ms_per_pass || read_planes < 0 || write_planes < 0 ||
+        read_planes + write_planes == 0)
+        return fail(ctx, QCD_EINVAL, "qcd_stream_mix: need two fields of this context, reps >= 1, plane counts >= 0 and a result pointer");
+    DEV(ctx, "qcd_stream_mix");
+    const size_t plane = (size_t)ctx->L.Vh * 2 * ctx->rsize / 16;            // 16-byte elements per plane of Vh complex numbers
+    if ((size_t)read_planes * plane * 16 > qcd_field_bytes(ctx, src->kind) || (size_t)write_planes * plane * 16 > qcd_field_bytes(ctx, dst->kind))
+        return fail(ctx, QCD_EINVAL, "qcd_stream_mix: more planes than the field holds");
+    if (overlaps(src->ptr, qcd_field_bytes(ctx, src->kind), dst->ptr, qcd_field_bytes(ctx, dst->kind)))
+        return fail(ctx, QCD_EINVAL, "qcd_stream_mix: src and dst overlap");
+    if (plane == 0) return fail(ctx, QCD_EINVAL, "qcd_stream_mix: lattice too small");
+    const size_t grid = (plane + MIX_BLOCK - 1) / MIX_BLOCK;
+    cudaEvent_t e0, e1;
+    CU(ctx, cudaEventCreate(&e0));
+    CU(ctx, cudaEventCreate(&e1));
+    cudaError_t err = cudaEventRecord(e0, ctx->stream);
+    for (int r = 0; r < reps && err == cudaSuccess; ++r) {
+        LaunchScope ls(ctx, QCD_K_MISC);
+        stream_mix_kernel<<<(unsigned)grid, MIX_BLOCK, 0, ctx->stream>>>((const double2 *)src->ptr, (double2 *)dst->ptr, plane, read_planes, write_planes);
+        err = cudaGetLastError();
+    }
+    if (err == cudaSuccess) err = cudaEventRecord(e1, ctx->stream);
+    if (err == cudaSuccess) err = cudaEventSynchronize(e1);
+    float ms = 0.f;
+    if (err == cudaSuccess) err = cudaEventElapsedTime(&ms, e0, e1);
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    if (err != cudaSuccess) return fail(ctx, QCD_ECUDA, "qcd_stream_mix: %s", cudaGetErrorString(err));
+    *ms_per_pass = (double)ms / reps;
+    return QCD_OK;
+}
+
 // ------------------------------------------------------------------------------------------
 // CG (n right-hand sides in lock step; qcd_cg_solve is n = 1)
 // ------------------------------------------------------------------------------------------

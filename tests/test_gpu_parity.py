@@ -398,6 +398,22 @@ def test_stream_read_hook(q, prec):
     assert np.array_equal(fU.download(), U)
     with pytest.raises(q.QcdError):
         ctx.qcd_stream_read_resident(fU, 0)
+    # the read / write mix: dst plane k = sum of the first `read_planes` planes of src, element by element
+    fD = ctx.field(q.QCD_GAUGE)
+    fD.buf.fill_(255)
+    assert ctx.qcd_stream_mix(fU, fD, 5, 2, 2) > 0.0
+    real = np.float64 if prec == 64 else np.float32
+    planes = fU.buf.cpu().numpy().view(real).reshape(72, -1)
+    got = fD.buf.cpu().numpy().view(real).reshape(72, -1)
+    want = planes[:5].astype(real).sum(axis=0, dtype=real) if prec == 64 else None
+    if prec == 64:                                                    # fp32 fields are summed as pairs of doubles: only the fp64 sum is meaningful
+        assert np.allclose(got[0], want, rtol=1e-14, atol=1e-14) and np.array_equal(got[0], got[1])
+    assert np.all(fD.buf.cpu().numpy().reshape(72, -1)[2:] == 255)    # planes beyond write_planes untouched
+    assert np.array_equal(fU.download(), U)
+    for bad in (lambda: ctx.qcd_stream_mix(fU, fU, 1, 1, 1), lambda: ctx.qcd_stream_mix(fU, fD, 73, 1, 1),
+                lambda: ctx.qcd_stream_mix(fU, fD, 0, 0, 1), lambda: ctx.qcd_stream_mix(fU, fD, 1, 1, 0)):
+        with pytest.raises(q.QcdError):
+            bad()
     other = q.Context(dims, prec)
     with pytest.raises(q.QcdError):
         other.qcd_stream_read(fU, 1)
