@@ -512,7 +512,9 @@ def test_cg_persistent_cluster_and_grid_shapes_agree(q, dims, links, eps, prec):
         assert info2["iters"] == info["iters"] and np.array_equal(fx.download(), x)          # bitwise reproducible
         out[cluster] = (info, x.astype(np.complex128))
     (ic, xc), (ig, xg) = out[True], out[False]
-    assert ic["converged"] and ig["converged"] and abs(ic["iters"] - ig["iters"]) <= 1
+    # the two shapes sum the per-block partials in different groupings; on the rounding plateau of 4^4 at 1e-10 (the oracle's own
+    # count moves by +-3 with its thread count) that shifts the stopping iteration by a few: reading R8 is the bound
+    assert ic["converged"] and ig["converged"] and iters_close(ic["iters"], ig["iters"])
     xo, oinfo = oracle.cg(dims, Ur.astype(ctx.cdtype), br.astype(ctx.cdtype), m, tol, 20000)
     for info, x in (out[True], out[False]):
         assert iters_close(info["iters"], oinfo["iters"]), (info, oinfo)
@@ -643,7 +645,7 @@ def test_cg_persistent_kernel(q, dims, links, eps, kind_name, prec):
     (i1, x1, l1), (i3, x3, l3) = out[1], out[3]
     assert i1["converged"] and i3["converged"]
     assert l3 == 2 and l1 >= 4 * i1["iters"]                       # init + ONE kernel for the whole solve
-    assert abs(i1["iters"] - i3["iters"]) <= 1, (i1, i3)
+    assert iters_close(i1["iters"], i3["iters"]), (i1, i3)          # reading R8 (the reduction orders differ)
     xo, oinfo = oracle.cg(dims, Ur.astype(ctx.cdtype), br.astype(ctx.cdtype), m, tol, 20000)
     assert iters_close(i3["iters"], oinfo["iters"]), (i3, oinfo)
     true = oracle.true_residual(dims, Ur, br, x3, m)
