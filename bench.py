@@ -104,7 +104,8 @@ def parse_args(argv=None):
     ap.add_argument("--nmulti", default="1,2,3,4,6,8", help="NMULTI values of --variants-only")
     ap.add_argument("--reps", type=int, default=10, help="timed launches per variant of --variants-only / --dslash-only")
     ap.add_argument("--kernel", type=int, default=0,
-                    help="qcd_set_dslash_variant for --variants-only (0 default choice, 4 staged kernel, 5 register kernel)")
+                    help="qcd_set_dslash_variant (A/B runs; 0 the library's choice, 1-3 block shapes of the one-vector kernel, 4 staged, "
+                         "5 register, 6/7 pair, 8 tile, 9 rolled kernel)")
     return ap.parse_args(argv)
 
 
@@ -298,6 +299,7 @@ def run_ours(args):
     prec = args.prec
     rsize = prec // 8
     ctx = q.Context(dims, prec, device=dev)
+    ctx.qcd_set_dslash_variant(args.kernel)                # 0 unless an A/B run asks for another block shape
     fU = ctx.field(q.QCD_GAUGE)
     fb = ctx.field(q.QCD_SPINOR_EVEN)
     fx = ctx.field(q.QCD_SPINOR_EVEN)
@@ -499,6 +501,7 @@ def run_dslash_only(args):
     fU = ctx.field(q.QCD_GAUGE).upload(U)
     fb = ctx.field(q.QCD_SPINOR_EVEN).upload(b)
     fo, fe = ctx.field(q.QCD_SPINOR_ODD), ctx.field(q.QCD_SPINOR_EVEN)
+    ctx.qcd_set_dslash_variant(args.kernel)
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     ctx.qcd_dslash_oe(fU, fo, fb)
     torch.cuda.synchronize()

@@ -305,13 +305,13 @@ def update_routine_report(q, torch, device, peak, dims=(48, 48, 48, 48), iters=5
 
 def config2_sweep_report(q, torch, device, peak, hbm_stream_gbs):
     """BASELINE.json configs[2]: "Dslash throughput sweep" at 32^4 in both precisions -- the block shapes of the one-vector
-    kernel that qcd_set_dslash_variant exposes (0: 128 threads x 4 resident blocks, the library's choice; 1: 64 x 8;
-    2: 256 x 2; 3: 128 x 3), D_oe launches replayed from a CUDA graph."""
+    kernel that qcd_set_dslash_variant exposes (0: 128 threads x 3 resident blocks, the library's choice; 1: 64 x 8;
+    2: 256 x 2; 3: 128 x 4), D_oe launches replayed from a CUDA graph."""
     import qcd_inputs
     cfg, U, b = qcd_inputs.config_inputs(2)
     dims = cfg["dims"]
     Vh = int(np.prod(dims)) // 2
-    names = {0: "128 threads x 4 blocks/SM (library's choice)", 1: "64 x 8", 2: "256 x 2", 3: "128 x 3"}
+    names = {0: "128 threads x 3 blocks/SM (library's choice for the plain Dslash)", 1: "64 x 8", 2: "256 x 2", 3: "128 x 4"}
     rows = []
     for prec in (64, 32):
         stream = torch.cuda.Stream(device=device)

@@ -264,10 +264,11 @@ qcd_status qcd_stream_mix(qcd_ctx *ctx, const qcd_field *src, qcd_field *dst, in
 
 /*
  * Tuning knob for the Dslash kernels (bench sweeps and A/B tests, Sec. 10):
- *   0 : the library's choice (128-thread blocks, 4 resident per SM for one vector; for several vectors
- *       the register kernel or the cp.async-staged kernel, whichever measured faster for that
- *       (precision, number of vectors, link storage))
- *   1, 2, 3 : one-vector kernel with 64 x 8, 256 x 2, 128 x 3 threads x resident blocks
+ *   0 : the library's choice (one vector: 128-thread blocks, 3 resident per SM for the plain Dslash on full links, 4 for the
+ *       kernels with the M epilogue and on two-row links; for several vectors the register kernel or the cp.async-staged
+ *       kernel, whichever measured faster for that (precision, number of vectors, link storage))
+ *   1, 2, 3 : one-vector kernel with 64 x 8, 256 x 2 threads x resident blocks, and 128 threads with the OTHER of 3 / 4 resident
+ *       blocks than the library's choice for that kernel
  *   4 : force the staged kernel (links prefetched through shared memory by cp.async)
  *   5 : force the register kernel
  *   6, 7 : force the pair kernel (two adjacent lanes per site, half of the vectors each, the link shared through the

@@ -35,10 +35,16 @@ template <> struct DslashCfg<float, 8> { enum { BLOCK = 128, MINB = 2 }; };
 //   * MODE 0 / 1 on full links want 3 blocks (168-register cap: the loads of the next direction are
 //     hoisted over the current one's FMAs): 1.44 -> 1.17-1.20 ms; on two-row links 4 blocks stay best.
 // fp32 kernels keep 4 blocks everywhere (their registers hold twice the loads already).
+// The plain one-vector Dslash on full links (MODE 0: D_oe, D_eo; the headline kernel) runs with THREE resident blocks (168-register
+// cap: ptxas hoists the next direction's loads over the current FMAs).  A/B in alternating runs of 40 launches (round 2, variant knob):
+// fp32 24^4 18.7 -> 16.6 us, 32^4 51.5 -> 47.4, 48^3 x 12 65.4 -> 60.7, 64^4 756.7 -> 739.3 (-2.3 %); fp64 24^4 31.0 -> 30.0, 32^4
+// 95.1 -> 94.1, 48^3 x 12 and 64^4 -0.1 ... -0.2 %.  The reducing kernel (MODE 2) is slower that way (fp32 CG iteration 1.850 -> 1.858 ms
+// with both kernels at 3 blocks although D_oe alone gains 0.022 ms) and keeps 4.
 template <typename T, int MODE, int NROW, int TG, int NRHS>
 struct DslashTune {
     enum { BLOCK = DslashCfg<T, NRHS>::BLOCK,
            MINB = (sizeof(T) == 8 && TG == 1 && NRHS == 1) ? (MODE == 2 ? 6 : (NROW == 3 ? 3 : DslashCfg<T, NRHS>::MINB))
+                : (NRHS == 1 && TG == 0 && MODE == 0 && NROW == 3) ? 3
                                                             : DslashCfg<T, NRHS>::MINB };
 };
 
@@ -200,7 +206,7 @@ static cudaError_t launch_nrhs(const DslashLaunch &d)
         switch (d.variant) {       // block-shape sweep of the headline kernel
         case 1: return launch_cfg<T, MODE, NROW, TG, 1, 64, 8>(d);
         case 2: return launch_cfg<T, MODE, NROW, TG, 1, 256, 2>(d);
-        case 3: return launch_cfg<T, MODE, NROW, TG, 1, 128, 3>(d);
+        case 3: return launch_cfg<T, MODE, NROW, TG, 1, 128, (DslashTune<T, MODE, NROW, TG, 1>::MINB == 3 ? 4 : 3)>(d);   // the OTHER of 3 / 4
         default: break;
         }
     }
