@@ -123,13 +123,18 @@ static cudaError_t launch_rolled(const DslashLaunch &d)
 
 // Staged kernel (links through shared memory by cp.async, dslash.cuh): ring of STAGE_DEPTH hops.
 enum { STAGE_DEPTH = 4 };
-template <typename T, int NRHS> struct StagedCfg { enum { BLOCK = 128, MINB = sizeof(T) == 8 ? (NRHS <= 4 ? 3 : 2) : (NRHS <= 4 ? 4 : 3) }; };
+// Resident blocks (register cap) of the staged kernel.  A/B of +-1 block at n = 3, 4 (round 2, alternating runs of 20 launches at 64^4):
+// fp64 full links n = 4 gains 4 % with 2 blocks (255 registers: 2.229 -> 2.138 ms); every other case is best, or within 2 %, as it is.
+template <typename T, int NRHS, int NROW = 3> struct StagedCfg {
+    enum { BLOCK = 128,
+           MINB = sizeof(T) == 8 ? ((NRHS == 4 && NROW == 3) ? 2 : (NRHS <= 4 ? 3 : 2)) : (NRHS <= 4 ? 4 : 3) };
+};
 
 template <typename T, int MODE, int NROW, int TG, int NRHS>
 static cudaError_t launch_staged(const DslashLaunch &d)
 {
     typedef typename Cplx<T>::type C;
-    enum { BLOCK = StagedCfg<T, NRHS>::BLOCK, MINB = StagedCfg<T, NRHS>::MINB };
+    enum { BLOCK = StagedCfg<T, NRHS, NROW>::BLOCK, MINB = (MODE == 0 ? (int)StagedCfg<T, NRHS, NROW>::MINB : (int)StagedCfg<T, NRHS>::MINB) };
     const size_t smem = (size_t)STAGE_DEPTH * 3 * NROW * BLOCK * sizeof(C);
     auto kernel = dslash_staged_kernel<T, MODE, NROW, TG, NRHS, BLOCK, MINB, STAGE_DEPTH>;
     // the attribute belongs to the (function, device) pair: set on every launch (a host-side table update, no device
