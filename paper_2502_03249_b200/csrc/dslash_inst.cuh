@@ -123,18 +123,39 @@ static cudaError_t launch_rolled(const DslashLaunch &d)
 
 // Staged kernel (links through shared memory by cp.async, dslash.cuh): ring of STAGE_DEPTH hops.
 enum { STAGE_DEPTH = 4 };
-// Resident blocks (register cap) of the staged kernel.  A/B of +-1 block at n = 3, 4 (round 2, alternating runs of 20 launches at 64^4):
-// fp64 full links n = 4 gains 4 % with 2 blocks (255 registers: 2.229 -> 2.138 ms); every other case is best, or within 2 %, as it is.
-template <typename T, int NRHS, int NROW = 3> struct StagedCfg {
-    enum { BLOCK = 128,
-           MINB = sizeof(T) == 8 ? ((NRHS == 4 && NROW == 3) ? 2 : (NRHS <= 4 ? 3 : 2)) : (NRHS <= 4 ? 4 : 3) };
-};
+template <typename T, int NRHS> struct StagedCfg { enum { BLOCK = 128, MINB = sizeof(T) == 8 ? (NRHS <= 4 ? 3 : 2) : (NRHS <= 4 ? 4 : 3) }; };
 
-template <typename T, int MODE, int NROW, int TG, int NRHS>
+// Kernel and register cap of the PLAIN multi-vector Dslash (MODE 0) per (precision, link storage, temporal gauge, n), where a sweep of
+// one resident block more / less for both kernels beat the general rule below by >= 4 % (round 2; 64^4, best of two runs of 10
+// launches per choice, all choices in one process sequence; profiles/README.md "register caps"): mostly the REGISTER kernel with one
+// block more than DslashCfg gives it -- more warps at a tighter cap beat the cp.async ring where both fit.
+//   kernel: 0 = the general rule, 1 = register kernel, 2 = staged kernel;  minb = resident blocks of 128 threads
+struct Mode0Choice { int kernel, minb; };
+template <typename T>
+constexpr Mode0Choice mode0_choice(int nrow, int tg, int n)
+{
+    if (sizeof(T) == 8) {
+        if (nrow == 3 && !tg && n >= 3 && n <= 6) return {1, 3};      // 1.84 -> 1.74 (n = 3), 2.14 -> 1.97 (4), 2.85 -> 2.70 ms (6)
+        if (nrow == 2 && !tg && n == 6) return {2, 3};                  // 2.50 -> 2.31 ms
+        if (nrow == 2 && n == 5) return {2, 2};                         // staged instead of register: 2.29 -> 2.01, in temporal gauge 2.24 -> 1.97 ms
+        if (!tg && n == 8) return {2, 2};                               // staged instead of register: full links 3.53 -> 3.32, two-row 3.31 -> 3.05 ms
+    } else {
+        if (nrow == 3 && !tg && n == 3) return {1, 5};                  // 0.982 -> 0.870 ms
+        if (nrow == 3 && !tg && n >= 4 && n <= 6) return {1, 4};        // 1.095 -> 1.009 (4), 1.487 -> 1.341 ms (6)
+        if (nrow == 2 && !tg && (n == 2 || n == 3)) return {1, 5};      // 0.612 -> 0.587, 0.777 -> 0.740 ms
+        if (nrow == 2 && !tg && n == 6) return {1, 4};                  // 1.293 -> 1.207 ms
+        if (nrow == 2 && !tg && n == 8) return {2, 4};                  // 1.670 -> 1.594 ms
+        if (nrow == 2 && tg && n == 2) return {2, 5};                   // 0.622 -> 0.561 ms
+        if (nrow == 2 && tg && n == 6) return {1, 4};                   // 1.206 -> 1.139 ms
+    }
+    return {0, 0};
+}
+
+template <typename T, int MODE, int NROW, int TG, int NRHS, int MINB_OVERRIDE = 0>
 static cudaError_t launch_staged(const DslashLaunch &d)
 {
     typedef typename Cplx<T>::type C;
-    enum { BLOCK = StagedCfg<T, NRHS, NROW>::BLOCK, MINB = (MODE == 0 ? (int)StagedCfg<T, NRHS, NROW>::MINB : (int)StagedCfg<T, NRHS>::MINB) };
+    enum { BLOCK = StagedCfg<T, NRHS>::BLOCK, MINB = MINB_OVERRIDE > 0 ? MINB_OVERRIDE : (int)StagedCfg<T, NRHS>::MINB };
     const size_t smem = (size_t)STAGE_DEPTH * 3 * NROW * BLOCK * sizeof(C);
     auto kernel = dslash_staged_kernel<T, MODE, NROW, TG, NRHS, BLOCK, MINB, STAGE_DEPTH>;
     // the attribute belongs to the (function, device) pair: set on every launch (a host-side table update, no device
@@ -200,6 +221,13 @@ static cudaError_t launch_nrhs(const DslashLaunch &d)
     // variant 4 forces the staged kernel, variant 5 the register kernel (A/B sweeps); otherwise the
     // staged kernel serves the (precision, NRHS, link rows) where it measured faster at 64^4
     // (profiles/README.md "staged vs register kernel"): fp64 n = 3, 4; fp32 n = 8, and n >= 4 on two-row links
+    if constexpr (MODE == 0 && NRHS >= 2) {
+        constexpr Mode0Choice c = mode0_choice<T>(NROW, TG, NRHS);
+        if (d.variant == 0) {
+            if constexpr (c.kernel == 1) return launch_cfg<T, MODE, NROW, TG, NRHS, 128, c.minb>(d);
+            if constexpr (c.kernel == 2) return launch_staged<T, MODE, NROW, TG, NRHS, c.minb>(d);
+        }
+    }
     if constexpr (MODE != 1) {
         // (the reducing kernel, MODE 2, on full links is 3-5 % faster as the register kernel at n = 3, 4: 2.35 / 2.71 ms
         // against 2.42 / 2.86 -- ncu shows the staged MODE 2 kernel requesting every link sector from the L2 twice)
