@@ -150,6 +150,22 @@ constexpr Mode0Choice mode0_choice(int nrow, int tg, int n)
     }
     return {0, 0};
 }
+// The same sweep for the REDUCING kernel (MODE 2), timed inside the lock-step CG iteration (CUDA events per launch): the round-1
+// choices are within 3 % of the best everywhere except here.  (The MODE 0 choices do not carry over: applied to MODE 2 they cost up
+// to 48 %.)
+template <typename T>
+constexpr Mode0Choice mode2_choice(int nrow, int tg, int n)
+{
+    if (sizeof(T) == 8) {
+        if (nrow == 2 && tg && n == 2) return {1, 4};                   // 1.513 -> 1.421 ms
+        if (nrow == 3 && !tg && n == 3) return {1, 3};                  // 2.378 -> 2.264 ms
+        if (nrow == 2 && tg && n == 4) return {1, 3};                   // 2.148 -> 2.062 ms
+    } else {
+        if (nrow == 2 && tg && n == 2) return {2, 5};                   // 0.767 -> 0.685 ms
+        if (nrow == 2 && !tg && n == 8) return {1, 3};                  // 2.684 -> 2.386 ms
+    }
+    return {0, 0};
+}
 
 template <typename T, int MODE, int NROW, int TG, int NRHS, int MINB_OVERRIDE = 0>
 static cudaError_t launch_staged(const DslashLaunch &d)
@@ -221,8 +237,8 @@ static cudaError_t launch_nrhs(const DslashLaunch &d)
     // variant 4 forces the staged kernel, variant 5 the register kernel (A/B sweeps); otherwise the
     // staged kernel serves the (precision, NRHS, link rows) where it measured faster at 64^4
     // (profiles/README.md "staged vs register kernel"): fp64 n = 3, 4; fp32 n = 8, and n >= 4 on two-row links
-    if constexpr (MODE == 0 && NRHS >= 2) {
-        constexpr Mode0Choice c = mode0_choice<T>(NROW, TG, NRHS);
+    if constexpr (MODE != 1 && NRHS >= 2) {
+        constexpr Mode0Choice c = MODE == 0 ? mode0_choice<T>(NROW, TG, NRHS) : mode2_choice<T>(NROW, TG, NRHS);
         if (d.variant == 0) {
             if constexpr (c.kernel == 1) return launch_cfg<T, MODE, NROW, TG, NRHS, 128, c.minb>(d);
             if constexpr (c.kernel == 2) return launch_staged<T, MODE, NROW, TG, NRHS, c.minb>(d);
