@@ -97,6 +97,9 @@ def parse_args(argv=None):
     ap.add_argument("--cg-only", action="store_true",
                     help="run only `--reps` full CG solves of BASELINE.json configs[--config] in --prec with the solver loop the "
                          "library picks; used for ncu captures of the small-lattice loops")
+    ap.add_argument("--cg-multi-only", action="store_true",
+                    help="run only `--reps` lock-step CG iterations over the first value of --nmulti right-hand sides at 64^4 (or --lattice), on "
+                         "full links and on two-row temporal-gauge links; used for ncu captures of the reducing multi-vector kernels")
     ap.add_argument("--config", type=int, default=4, choices=(0, 1, 2, 3, 4), help="BASELINE.json config of --dslash-only / --cg-only")
     ap.add_argument("--prec", type=int, default=64, choices=(64, 32),
                     help="precision of --variants-only / --dslash-only, and of the timed CG iterations (32: the fp32 path of "
@@ -205,7 +208,7 @@ def free_port() -> int:
 def respawn_under_torchrun(args, argv) -> int | None:
     """`python bench.py --gpus N` with N > 1 and no torchrun environment: launch N ranks (one per GPU) of this very
     command under torch.distributed.run and return its exit code; None when no re-launch is needed."""
-    if args.gpus <= 1 or "WORLD_SIZE" in os.environ or args.variants_only or args.dslash_only or args.cg_only:
+    if args.gpus <= 1 or "WORLD_SIZE" in os.environ or args.variants_only or args.dslash_only or args.cg_only or args.cg_multi_only:
         return None
     cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(args.gpus),
            "--master-addr", "127.0.0.1", "--master-port", str(free_port()), os.path.abspath(__file__)] + list(argv)
@@ -543,6 +546,22 @@ def run_cg_only(args):
         ctx.close()
 
 
+def run_cg_multi_only(args):
+    """Lock-step CG iterations alone (bench_reports.cg_multi_report for one n): the command the captures of the multi-vector
+    reducing kernels under profiles/ are taken with."""
+    import torch
+    import bench_reports
+    import paper_2502_03249_b200 as q
+    dims = tuple(int(v) for v in args.lattice.split(",")) if args.lattice else (64, 64, 64, 64)
+    cfg, U, _ = make_inputs(dims)
+    n = int(args.nmulti.split(",")[0])
+    ctx = q.Context(dims, args.prec)
+    fU = ctx.field(q.QCD_GAUGE).upload(U)
+    rows = bench_reports.cg_multi_report(q, torch, ctx.device, dims, args.prec, fU, cfg["m"], ns=(n,), iters=max(args.reps, 1))
+    print(json.dumps({"cg_multi_only": True, "lattice": list(dims), "prec": args.prec, "rows": rows}), flush=True)
+    ctx.close()
+
+
 def main(argv=None):
     argv = sys.argv[1:] if argv is None else argv
     args = parse_args(argv)
@@ -555,6 +574,8 @@ def main(argv=None):
         run_dslash_only(args)
     elif args.cg_only:
         run_cg_only(args)
+    elif args.cg_multi_only:
+        run_cg_multi_only(args)
     elif args.impl == "reference":
         run_reference(args)
     else:
