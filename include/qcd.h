@@ -342,6 +342,37 @@ qcd_status qcd_cg_timeline_read(qcd_ctx *ctx, unsigned long long *host_out, int 
  * double accumulation); synchronises.  Used by tests and by callers that need norms. */
 qcd_status qcd_re_dot(qcd_ctx *ctx, const qcd_field *a, const qcd_field *b, double *result);
 
+/*
+ * The same dot product for callers that cannot allocate (code under CUDA graph capture, tight serving
+ * loops, harnesses that forbid cudaMalloc): no qcd_ctx (qcd_init allocates), no cudaMalloc / cudaFree and no
+ * allocating library routine, at set-up or later.  The reduction scratch (stage-1 partial sums + last-block
+ * tickets, "dot product involving global reductions") is a file-scope __device__ array of
+ * QCD_RE_DOT_STATIC_SCRATCH_BYTES (198 400 bytes) that every GPU loading the library holds until the
+ * process exits; it bounds the size of one call:
+ *       n_reals <= QCD_RE_DOT_STATIC_MAX_REALS = 50 331 648  (one 64^4 half-field: 3 colours x 2 reals x 64^4 / 2)
+ * in both precisions.  A larger n_reals is rejected with QCD_EINVAL; use qcd_re_dot on a context there.
+ *   a_dev, b_dev : DEVICE pointers (of the current device) to n_reals reals of `precision` (64: double,
+ *                  32: float), e.g. two half-fields in the device layout; 16-byte aligned, n_reals * size a
+ *                  multiple of 16 bytes; read only, may alias each other
+ *   cuda_stream  : a cudaStream_t of the current device, borrowed (NULL = legacy default stream)
+ *   result_dev   : DEVICE pointer to one double, 8-byte aligned, caller-owned: receives
+ *                  sum_i a[i] b[i] (products and sums in double, the summation order of qcd_re_dot: the
+ *                  two calls return the same value on the same data); 0.0 for n_reals = 0
+ *   errbuf       : HOST buffer of errbuf_bytes for the message of a failure ("" on success); may be NULL
+ * Asynchronous: enqueues one 1.5 KB memset of the tickets and one kernel on cuda_stream and returns; the
+ * result is valid once that work has completed.  The first call on each device also resolves the array's
+ * device address (cudaGetSymbolAddress, which may load the module): make it before capturing a graph.
+ * SHARED SCRATCH: every call, from every thread and stream, uses the same array, which keeps the last call's
+ * contents (the tickets are cleared by every call).  Calls that may overlap on the GPU -- different streams
+ * without an ordering between them -- RACE on it and return garbage: order them.  Calls on one stream are safe.
+ * Errors: QCD_EINVAL (NULL, precision, alignment, n_reals beyond the maximum, a pointer that is not memory of
+ * the current device), QCD_ECUDA (no device -- there is no CPU fallback -- or a CUDA failure).
+ */
+#define QCD_RE_DOT_STATIC_MAX_REALS 50331648
+#define QCD_RE_DOT_STATIC_SCRATCH_BYTES 198400
+qcd_status qcd_re_dot_static(const void *a_dev, const void *b_dev, size_t n_reals, int precision,
+                             void *cuda_stream, double *result_dev, char *errbuf, size_t errbuf_bytes);
+
 /* =========================================================================================
  * Variants: the paper's Dslash optimisations (Sec. 4.3) and mixed precision.
  * ========================================================================================= */

@@ -25,6 +25,7 @@ QCD_OK, QCD_EINVAL, QCD_ENOMEM, QCD_ECUDA, QCD_ENOTCONVERGED, QCD_EBREAKDOWN = r
 QCD_SPINOR_EVEN, QCD_SPINOR_ODD, QCD_SPINOR_FULL, QCD_GAUGE, QCD_GAUGE_2ROW, QCD_COLOUR_MATRIX = range(6)
 QCD_MAX_RHS = 8
 QCD_K_DSLASH, QCD_K_DSLASH_EPI, QCD_K_UPDATE_XR, QCD_K_UPDATE_P, QCD_K_MISC = range(5)
+QCD_RE_DOT_STATIC_MAX_REALS = 50331648      # include/qcd.h: one 64^4 half-field
 
 # every symbol include/qcd.h declares
 SYMBOLS = [
@@ -33,7 +34,7 @@ SYMBOLS = [
     "qcd_field_download", "qcd_set_workspace", "qcd_dslash_eo", "qcd_dslash_oe", "qcd_apply_M",
     "qcd_cg_solve", "qcd_cg_begin", "qcd_cg_iterate", "qcd_cg_poll", "qcd_cg_finish",
     "qcd_cg_solve_host", "qcd_profile_enable", "qcd_profile_read", "qcd_launch_count",
-    "qcd_set_dslash_variant", "qcd_set_traversal_chunk", "qcd_set_cg_loop", "qcd_last_cg_loop", "qcd_last_cg_cluster", "qcd_set_cg_cluster", "qcd_cg_timeline_enable", "qcd_cg_timeline_read", "qcd_re_dot", "qcd_stream_read", "qcd_stream_read_resident", "qcd_stream_mix", "qcd_cg_history",
+    "qcd_set_dslash_variant", "qcd_set_traversal_chunk", "qcd_set_cg_loop", "qcd_last_cg_loop", "qcd_last_cg_cluster", "qcd_set_cg_cluster", "qcd_cg_timeline_enable", "qcd_cg_timeline_read", "qcd_re_dot", "qcd_re_dot_static", "qcd_stream_read", "qcd_stream_read_resident", "qcd_stream_mix", "qcd_cg_history",
     # variants and mixed precision
     "qcd_gauge_compress", "qcd_gauge_fix_temporal", "qcd_gauge_set_temporal_unit", "qcd_spinor_rotate",
     "qcd_workspace_bytes_multi", "qcd_dslash_eo_multi", "qcd_dslash_oe_multi", "qcd_cg_solve_multi",
@@ -104,6 +105,7 @@ def load_library() -> ctypes.CDLL:
         "qcd_cg_timeline_enable": (ci, [vp, ci]),
         "qcd_cg_timeline_read": (ci, [vp, P(ctypes.c_ulonglong), ci, P(ci)]),
         "qcd_re_dot": (ci, [vp, vp, vp, P(cd)]),
+        "qcd_re_dot_static": (ci, [vp, vp, sz, ci, vp, vp, ctypes.c_char_p, sz]),
         "qcd_stream_read": (ci, [vp, vp, ci, P(cd)]),
         "qcd_stream_read_resident": (ci, [vp, vp, ci, P(cd)]),
         "qcd_stream_mix": (ci, [vp, vp, vp, ci, ci, ci, P(cd)]),
@@ -126,6 +128,17 @@ def load_library() -> ctypes.CDLL:
         fn.restype, fn.argtypes = res, args
     _LIB = lib
     return lib
+
+
+def qcd_re_dot_static(a_dev: int, b_dev: int, n_reals: int, precision: int, cuda_stream: int, result_dev: int) -> None:
+    """The allocation-free dot product (include/qcd.h): device addresses in, one double written at result_dev on
+    `cuda_stream`; asynchronous.  No context, no cudaMalloc; n_reals <= QCD_RE_DOT_STATIC_MAX_REALS."""
+    lib = load_library()
+    err = ctypes.create_string_buffer(512)
+    s = lib.qcd_re_dot_static(ctypes.c_void_p(a_dev), ctypes.c_void_p(b_dev), n_reals, precision,
+                              ctypes.c_void_p(cuda_stream), ctypes.c_void_p(result_dev), err, len(err))
+    if s != QCD_OK:
+        raise QcdError(s, "qcd_re_dot_static", err.value.decode())
 
 
 def _torch():
