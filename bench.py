@@ -108,7 +108,9 @@ def parse_args(argv=None):
     ap.add_argument("--reps", type=int, default=10, help="timed launches per variant of --variants-only / --dslash-only")
     ap.add_argument("--kernel", type=int, default=0,
                     help="qcd_set_dslash_variant (A/B runs; 0 the library's choice, 1-3 block shapes of the one-vector kernel, 4 staged, "
-                         "5 register, 6/7 pair, 8 tile, 9 rolled kernel)")
+                         "5 register, 6/7 pair, 8 tile, 9 rolled, 10 bulk-copy kernel)")
+    ap.add_argument("--stream-bulk", action="store_true",
+                    help="run only the qcd_stream_bulk sweep (requested bytes per second through the TMA copy engine, 64^4 gauge field) and print it")
     return ap.parse_args(argv)
 
 
@@ -208,7 +210,7 @@ def free_port() -> int:
 def respawn_under_torchrun(args, argv) -> int | None:
     """`python bench.py --gpus N` with N > 1 and no torchrun environment: launch N ranks (one per GPU) of this very
     command under torch.distributed.run and return its exit code; None when no re-launch is needed."""
-    if args.gpus <= 1 or "WORLD_SIZE" in os.environ or args.variants_only or args.dslash_only or args.cg_only or args.cg_multi_only:
+    if args.gpus <= 1 or "WORLD_SIZE" in os.environ or args.variants_only or args.dslash_only or args.cg_only or args.cg_multi_only or args.stream_bulk:
         return None
     cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(args.gpus),
            "--master-addr", "127.0.0.1", "--master-port", str(free_port()), os.path.abspath(__file__)] + list(argv)
@@ -562,6 +564,33 @@ def run_cg_multi_only(args):
     ctx.close()
 
 
+def run_stream_bulk(args):
+    """qcd_stream_bulk sweep alone (rank 0, one GPU): the rate at which the SMs take in requested bytes through the TMA copy engine, for
+    the box shapes and ring depths of the multi-vector Dslash, beside the LSU read stream over the same field."""
+    import torch
+    import paper_2502_03249_b200 as q
+    dims = tuple(int(v) for v in args.lattice.split(",")) if args.lattice else (64, 64, 64, 64)
+    ctx = q.Context(dims, 64, workspace=False)
+    fU = ctx.field(q.QCD_GAUGE)
+    fU.buf.view(torch.float64).normal_()
+    groups = int(np.prod(dims)) // 2 // 128
+    rows_out = []
+    ctx.qcd_stream_read(fU, 2)
+    lsu = fU.nbytes / ctx.qcd_stream_read(fU, args.reps) / 1e6
+    # (rows per copy, copies per stage, stages, producer warps): one link box = 9 rows; a vector box = 3 rows
+    for rows, copies, stages, producers in ((9, 1, 4, 1), (9, 3, 3, 3), (3, 3, 4, 1), (3, 7, 4, 1), (3, 7, 4, 4), (21, 1, 4, 1), (3, 11, 3, 1), (3, 11, 3, 2),
+                                            (3, 11, 3, 4), (11, 3, 3, 1), (11, 3, 3, 3), (33, 1, 3, 1), (1, 33, 3, 4), (1, 9, 8, 4)):
+        ctx.qcd_stream_bulk(fU, rows, copies, 8, stages, producers, 1)
+        ms = ctx.qcd_stream_bulk(fU, rows, copies, 8, stages, producers, args.reps)
+        req = groups * 8 * copies * rows * 2048
+        hbm = groups * min(72, 8 * copies * rows) * 2048
+        rows_out.append({"rows_per_copy": rows, "copies_per_stage": copies, "stage_kb": rows * copies * 2, "stages": stages, "producer_warps": producers,
+                         "ms": round(ms, 4), "requested_tbs": round(req / ms / 1e9, 2), "of_which_hbm_tbs": round(hbm / ms / 1e9, 2),
+                         "us_per_stage_and_sm": round(ms * 1e3 / (groups * 8 / 148), 3)})
+    print(json.dumps({"stream_bulk": rows_out, "lsu_read_stream_gbs": round(lsu, 1), "lattice": list(dims), "gpu_launches": ctx.qcd_launch_count()}), flush=True)
+    ctx.close()
+
+
 def main(argv=None):
     argv = sys.argv[1:] if argv is None else argv
     args = parse_args(argv)
@@ -576,6 +605,8 @@ def main(argv=None):
         run_cg_only(args)
     elif args.cg_multi_only:
         run_cg_multi_only(args)
+    elif args.stream_bulk:
+        run_stream_bulk(args)
     elif args.impl == "reference":
         run_reference(args)
     else:

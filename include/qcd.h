@@ -261,6 +261,19 @@ qcd_status qcd_stream_read_resident(qcd_ctx *ctx, const qcd_field *f, int passes
  * planes than a field holds, reps < 1), QCD_ECUDA.
  */
 qcd_status qcd_stream_mix(qcd_ctx *ctx, const qcd_field *src, qcd_field *dst, int read_planes, int write_planes, int reps, double *ms_per_pass);
+/*
+ * Streaming ceiling of the BULK-COPY (TMA) path (measurement hook; precision-64 contexts, the NMULTI kernels): one block
+ * per SM walks the planes of src (Vh complex numbers each) in groups of 128 consecutive sites; for each group, `hops` times, `producers`
+ * warps (1 .. 4) issue `copies` tensor-map copies of `rows` planes x 128 sites (2 KB per plane) into a ring of `stages` shared-memory
+ * stages (stages x copies x rows x 2 KB must fit a block's shared memory), and four consumer warps read every byte back from shared
+ * memory.  Plane rows wrap around inside the field, so once hops x copies x rows exceeds the field's planes the re-reads are L2 hits,
+ * like the neighbour gathers of a Dslash.  `reps` passes, CUDA events on the context stream, synchronises; *ms_per_pass is the average;
+ * requested bytes per pass = (Vh / 128) * hops * copies * rows * 2048.  What it measures: the rate at which a SM takes in requested bytes
+ * through the copy engine (about 15 TB/s on the chip), against the 9 - 11 TB/s of every LSU-fed Dslash kernel.
+ * Errors: QCD_EINVAL (NULL, foreign field, precision 32, a range above, Vh not a multiple of 128), QCD_ECUDA.
+ */
+qcd_status qcd_stream_bulk(qcd_ctx *ctx, const qcd_field *src, int rows, int copies, int hops, int stages, int producers, int reps,
+                           double *ms_per_pass);
 
 /*
  * Tuning knob for the Dslash kernels (bench sweeps and A/B tests, Sec. 10):
@@ -277,7 +290,11 @@ qcd_status qcd_stream_mix(qcd_ctx *ctx, const qcd_field *src, qcd_field *dst, in
  *   8 : force the register kernel with the x0 / x1 neighbour rows of a block staged in shared memory; applies to 4 or 8
  *       vectors on lattices where 128 consecutive sites are whole x0-rows of one (x2, x3) plane, otherwise the library's choice
  *   9 : force the kernel whose loop over the four directions is not unrolled (3 .. 8 vectors)
- * 6 .. 9 are the round-2 experiments (profiles/README.md); none measured faster than the library's choice.
+ *  10 : force the bulk-copy kernel (warp-specialised: producer warps feed a shared-memory ring with tensor-map copies, consumer
+ *       warps compute; plain Dslash of 2 .. 8 vectors on lattices where 128 consecutive sites are whole x0-rows of one (x2, x3)
+ *       plane, otherwise the library's choice)
+ * 6 .. 10 are the round-2 experiments (profiles/README.md); none measured faster than the library's choice (10 is on a
+ * par with it for 6 and 8 vectors on full fp64 links and slower elsewhere).
  * Every variant computes the same result (bitwise).  Unknown variants -> QCD_EINVAL.
  */
 qcd_status qcd_set_dslash_variant(qcd_ctx *ctx, int variant);

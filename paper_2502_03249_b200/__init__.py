@@ -34,7 +34,7 @@ SYMBOLS = [
     "qcd_field_download", "qcd_set_workspace", "qcd_dslash_eo", "qcd_dslash_oe", "qcd_apply_M",
     "qcd_cg_solve", "qcd_cg_begin", "qcd_cg_iterate", "qcd_cg_poll", "qcd_cg_finish",
     "qcd_cg_solve_host", "qcd_profile_enable", "qcd_profile_read", "qcd_launch_count",
-    "qcd_set_dslash_variant", "qcd_set_traversal_chunk", "qcd_set_cg_loop", "qcd_last_cg_loop", "qcd_last_cg_cluster", "qcd_set_cg_cluster", "qcd_cg_timeline_enable", "qcd_cg_timeline_read", "qcd_re_dot", "qcd_re_dot_static", "qcd_stream_read", "qcd_stream_read_resident", "qcd_stream_mix", "qcd_cg_history",
+    "qcd_set_dslash_variant", "qcd_set_traversal_chunk", "qcd_set_cg_loop", "qcd_last_cg_loop", "qcd_last_cg_cluster", "qcd_set_cg_cluster", "qcd_cg_timeline_enable", "qcd_cg_timeline_read", "qcd_re_dot", "qcd_re_dot_static", "qcd_stream_read", "qcd_stream_read_resident", "qcd_stream_mix", "qcd_stream_bulk", "qcd_cg_history",
     # variants and mixed precision
     "qcd_gauge_compress", "qcd_gauge_fix_temporal", "qcd_gauge_set_temporal_unit", "qcd_spinor_rotate",
     "qcd_workspace_bytes_multi", "qcd_dslash_eo_multi", "qcd_dslash_oe_multi", "qcd_cg_solve_multi",
@@ -109,6 +109,7 @@ def load_library() -> ctypes.CDLL:
         "qcd_stream_read": (ci, [vp, vp, ci, P(cd)]),
         "qcd_stream_read_resident": (ci, [vp, vp, ci, P(cd)]),
         "qcd_stream_mix": (ci, [vp, vp, vp, ci, ci, ci, P(cd)]),
+        "qcd_stream_bulk": (ci, [vp, vp, ci, ci, ci, ci, ci, ci, P(cd)]),
         "qcd_cg_history": (ci, [vp, ci, P(cd), ci, P(ci)]),
         "qcd_gauge_compress": (ci, [vp, vp, vp]),
         "qcd_gauge_fix_temporal": (ci, [vp, vp, vp, vp]),
@@ -369,6 +370,12 @@ class Context:
         ms = ctypes.c_double()
         self._check(self.lib.qcd_stream_mix(self.handle, src.handle, dst.handle, int(read_planes), int(write_planes), int(reps),
                                             ctypes.byref(ms)), "qcd_stream_mix")
+        return ms.value
+
+    def qcd_stream_bulk(self, src: Field, rows: int, copies: int, hops: int, stages: int, producers: int, reps: int) -> float:
+        ms = ctypes.c_double()
+        self._check(self.lib.qcd_stream_bulk(self.handle, src.handle, int(rows), int(copies), int(hops), int(stages), int(producers), int(reps),
+                                             ctypes.byref(ms)), "qcd_stream_bulk")
         return ms.value
 
     # ---- variants -------------------------------------------------------

@@ -2,6 +2,7 @@
 // four dslash_*.cu translation units, each of which instantiates launch_dslash_impl once.
 #pragma once
 #include "dslash.cuh"
+#include "dslash_bulk.cuh"
 #include "dslash_launch.h"
 
 namespace qcd {
@@ -215,9 +216,50 @@ static cudaError_t launch_pair(const DslashLaunch &d)
     return cudaGetLastError();
 }
 
+// Bulk-copy kernel (dslash_bulk.cuh): needs a block's 128 sites to be whole x0-rows of one (x2, x3) plane.
+static inline bool bulk_eligible(const Lattice &L) { return tile_eligible(L, BULK_SITES) && L.Vh % BULK_SITES == 0; }
+template <typename T, int MODE, int NROW, int TG, int NRHS>
+static cudaError_t launch_bulk(const DslashLaunch &d)
+{
+    typedef typename Cplx<T>::type C;
+    typedef BulkStage<T, NROW, NRHS> St;
+    int dev = 0, sms = 0, max_smem = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&max_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
+    if (e != cudaSuccess) return e;
+    int stages = (max_smem - 1024) / (int)St::BYTES;
+    if (stages > BULK_RING_MAX) stages = BULK_RING_MAX;
+    if (stages < 2) return cudaErrorInvalidValue;
+    const size_t smem = (size_t)stages * St::BYTES;
+    auto kernel = dslash_bulk_kernel<T, MODE, NROW, TG, NRHS>;
+    e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    DslashArgs<T, NRHS> a;
+    a.L = d.L; a.parity = d.parity; a.U = (const C *)d.U;
+    for (int r = 0; r < NRHS; ++r) { a.in[r] = (const C *)d.in[r]; a.out[r] = (C *)d.out[r]; a.v[r] = (const C *)d.v[r]; }
+    a.m2 = (T)d.m2; a.partials = d.partials; a.scal = d.scal; a.check_flag = d.check_flag; a.chunks = 1;
+    BulkMaps<NRHS> maps;
+    const bool f64 = sizeof(T) == 8;
+    e = encode_plane_map(&maps.U, f64, d.U, 2ull * d.L.Vh, 24ull * NROW, (unsigned long long)d.L.Vh * sizeof(C), 2 * BULK_SITES, 3 * NROW);
+    for (int r = 0; r < NRHS && e == cudaSuccess; ++r)
+        e = encode_plane_map(&maps.in[r], f64, d.in[r], 2ull * d.L.Vh, 3, (unsigned long long)d.L.Vh * sizeof(C), 2 * BULK_SITES, 3);
+    if (e != cudaSuccess) return e;
+    const int ngroups = d.L.Vh / BULK_SITES;
+    const int grid = ngroups < sms ? ngroups : sms;
+    kernel<<<grid, BULK_BLOCK, smem, d.stream>>>(a, maps, stages, ngroups);
+    return cudaGetLastError();
+}
+
 template <typename T, int MODE, int NROW, int TG, int NRHS>
 static cudaError_t launch_nrhs(const DslashLaunch &d)
 {
+    // variant 10 forces the bulk-copy (TMA) kernel where the lattice allows it.  Not dispatched: at 64^4 on full fp64 links it is on a par
+    // with the register kernel for 6 and 8 vectors (2.67 - 2.70 / 3.41 - 3.67 ms against 2.75 - 2.89 / 3.55 - 3.57 from run to run), 11 % slower for 7
+    // (the two consumer halves hold 4 and 3 vectors) and slower everywhere else (profiles/r02_bulk_copy_kernel.md)
+    if constexpr (MODE == 0 && NRHS >= 2) {
+        if (d.variant == 10 && bulk_eligible(d.L)) return launch_bulk<T, MODE, NROW, TG, NRHS>(d);
+    }
     // variants 6 / 7 force the pair kernel at a 168- / 128-register cap (A/B sweeps); it needs an even number of vectors
     // and a volume of whole 64-site blocks
     // variant 9 forces the rolled kernel (direction loop not unrolled: a quarter of the code; dslash.cuh)

@@ -4,6 +4,7 @@
 // followed by all odd sites"): idx = x0 + N0 (x1 + N1 (x2 + N2 x3)), cb = idx >> 1, every
 // complex component of a field is one plane of Vh contiguous (re, im) pairs.
 #pragma once
+#include <cuda.h>
 #include <cuda_runtime.h>
 #include <stdint.h>
 
@@ -124,6 +125,52 @@ __device__ __forceinline__ void cp_async_plain(float2 *smem_dst, const float2 *s
     const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
     asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" :: "r"(d), "l"(src) : "memory");
 }
+// ---- mbarrier + bulk asynchronous copies (cp.async.bulk: the TMA engine moves a contiguous run global -> shared and
+// signals an mbarrier with the bytes it wrote; no thread holds a register or an LSU miss entry for the data in flight) ----
+__device__ __forceinline__ unsigned smem_addr(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned long long *bar, unsigned count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" :: "r"(smem_addr(bar)), "r"(count) : "memory");
+}
+// after the inits, before any other thread or the async proxy touches the barriers
+__device__ __forceinline__ void mbar_init_fence()
+{
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_arrive(unsigned long long *bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" :: "r"(smem_addr(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(unsigned long long *bar, unsigned bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" :: "r"(smem_addr(bar)), "r"(bytes) : "memory");
+}
+// wait until the phase of parity `parity` has completed; a wait that never completes (a byte-count bug) traps instead of hanging the GPU
+__device__ __forceinline__ void mbar_wait(unsigned long long *bar, unsigned parity)
+{
+    const unsigned a = smem_addr(bar);
+    unsigned ok = 0;
+    for (unsigned spins = 0; !ok; ++spins) {
+        asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+                     : "=r"(ok) : "r"(a), "r"(parity) : "memory");
+        if (spins > (1u << 26)) __trap();
+    }
+}
+// `bytes` (a multiple of 16) from 16-byte aligned global memory to 16-byte aligned shared memory; completion is counted on `bar`
+__device__ __forceinline__ void bulk_copy_g2s(void *smem_dst, const void *src, unsigned bytes, unsigned long long *bar, uint64_t pol)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;"
+                 :: "r"(smem_addr(smem_dst)), "l"(src), "r"(bytes), "r"(smem_addr(bar)), "l"(pol) : "memory");
+}
+
+// one BOX of a 2-d tensor map (inner coordinate c0, outer c1) -> shared memory; the box shape is fixed by the map
+__device__ __forceinline__ void tensor_copy_g2s(void *smem_dst, const void *tmap, int c0, int c1, unsigned long long *bar, uint64_t pol)
+{
+    asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1, {%2, %3}], [%4], %5;"
+                 :: "r"(smem_addr(smem_dst)), "l"(tmap), "r"(c0), "r"(c1), "r"(smem_addr(bar)), "l"(pol) : "memory");
+}
+
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 // wait until at most `pending` of this thread's most recent groups are still in flight
 // (the operand must be an immediate: the switch folds once the caller's loop is unrolled)
@@ -203,6 +250,31 @@ __device__ __forceinline__ SiteGeom site_geometry(const Lattice &L, int parity, 
     g.sb[3] = (x3 == 0) ? e3 : -e3;                  // backward hop across the time seam
     g.x3 = x3;
     return g;
+}
+
+// Host: tensor map of `planes` rows of `row_elems` elements (8-byte doubles or 4-byte floats), rows `row_stride_bytes` apart,
+// with a box of box_rows x box_elems.  cuTensorMapEncodeTiled is taken from the driver through the runtime (no libcuda link).
+static inline cudaError_t encode_plane_map(CUtensorMap *map, bool f64, const void *base, unsigned long long row_elems, unsigned long long planes,
+                                           unsigned long long row_stride_bytes, unsigned box_elems, unsigned box_rows)
+{
+    typedef CUresult (*encode_fn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *, const cuuint32_t *,
+                                  const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+    static encode_fn fn = nullptr;
+    if (!fn) {
+        void *p = nullptr;
+        cudaDriverEntryPointQueryResult qr;
+        const cudaError_t e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qr);
+        if (e != cudaSuccess) return e;
+        if (qr != cudaDriverEntryPointSuccess || !p) return cudaErrorNotSupported;
+        fn = (encode_fn)p;
+    }
+    const cuuint64_t gdim[2] = {row_elems, planes};
+    const cuuint64_t gstride[1] = {row_stride_bytes};
+    const cuuint32_t box[2] = {box_elems, box_rows};
+    const cuuint32_t estr[2] = {1, 1};
+    const CUresult r = fn(map, f64 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, const_cast<void *>(base), gdim, gstride, box, estr,
+                          CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    return r == CUDA_SUCCESS ? cudaSuccess : cudaErrorInvalidValue;
 }
 
 } // namespace qcd

@@ -9,6 +9,7 @@
 #include <math.h>
 #include <stdint.h>
 #include <stdio.h>
+#include <stdlib.h>
 #include <string.h>
 
 #include <new>
@@ -418,7 +419,7 @@ extern "C" qcd_status qcd_cg_timeline_read(qcd_ctx *ctx, unsigned long long *hos
 extern "C" qcd_status qcd_set_dslash_variant(qcd_ctx *ctx, int variant)
 {
     if (!ctx) return QCD_EINVAL;
-    if (variant < 0 || variant > 9) return fail(ctx, QCD_EINVAL, "qcd_set_dslash_variant: unknown variant");
+    if (variant < 0 || variant > 10) return fail(ctx, QCD_EINVAL, "qcd_set_dslash_variant: unknown variant");
     ctx->variant = variant;
     return QCD_OK;
 }
@@ -744,6 +745,50 @@ extern "C" qcd_status qcd_stream_mix(qcd_ctx *ctx, const qcd_field *src, qcd_fie
     cudaEventDestroy(e0);
     cudaEventDestroy(e1);
     if (err != cudaSuccess) return fail(ctx, QCD_ECUDA, "qcd_stream_mix: %s", cudaGetErrorString(err));
+    *ms_per_pass = (double)ms / reps;
+    return QCD_OK;
+}
+
+// Streaming ceiling of the bulk-copy (TMA) path (measure_kernels.cuh).
+extern "C" qcd_status qcd_stream_bulk(qcd_ctx *ctx, const qcd_field *src, int rows, int copies, int hops, int stages, int producers,
+                                      int reps, double *ms_per_pass)
+{
+    if (!ctx) return QCD_EINVAL;
+    if (!src || src->ctx != ctx || !ms_per_pass || reps < 1 || rows < 1 || rows > 256 || copies < 1 || hops < 1 || stages < 2 || stages > BULK_MAX_STAGES ||
+        producers < 1 || producers > BULK_MAX_PRODUCERS)
+        return fail(ctx, QCD_EINVAL, "qcd_stream_bulk: need a field of this context, 1 <= rows <= 256, copies >= 1, hops >= 1, 2 <= stages <= 12, 1 <= producers <= 4, "
+                                     "reps >= 1 and a result pointer");
+    if (ctx->prec != 64) return fail(ctx, QCD_EINVAL, "qcd_stream_bulk: the hook reads 16-byte elements of a precision-64 context");
+    DEV(ctx, "qcd_stream_bulk");
+    const size_t plane = (size_t)ctx->L.Vh;                                  // complex doubles per plane
+    const int nplanes = (int)(qcd_field_bytes(ctx, src->kind) / (plane * 16));
+    if (plane % BULK_RUN || rows > nplanes) return fail(ctx, QCD_EINVAL, "qcd_stream_bulk: a plane must be a multiple of 128 sites and hold `rows` planes");
+    const size_t smem = (size_t)stages * rows * copies * BULK_RUN * 16;
+    int max_smem = 0, sms = 0;
+    CU(ctx, cudaDeviceGetAttribute(&max_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, ctx->dev));
+    CU(ctx, cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, ctx->dev));
+    if (smem > (size_t)max_smem) return fail(ctx, QCD_EINVAL, "qcd_stream_bulk: stages x rows x copies x 2 KB exceeds the shared memory of a block");
+    CUtensorMap map;
+    CU(ctx, encode_plane_map(&map, true, src->ptr, plane * 2, nplanes, plane * 16, BULK_RUN * 2, rows));
+    CU(ctx, cudaFuncSetAttribute(stream_bulk_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    const size_t ngroups = plane / BULK_RUN;
+    const unsigned grid = (unsigned)(ngroups < (size_t)sms ? ngroups : (size_t)sms);
+    cudaEvent_t e0, e1;
+    CU(ctx, cudaEventCreate(&e0));
+    CU(ctx, cudaEventCreate(&e1));
+    cudaError_t err = cudaEventRecord(e0, ctx->stream);
+    for (int r = 0; r < reps && err == cudaSuccess; ++r) {
+        LaunchScope ls(ctx, QCD_K_MISC);
+        stream_bulk_kernel<<<grid, BULK_CONSUMERS + 32 * producers, smem, ctx->stream>>>(map, nplanes, rows, copies, hops, stages, ngroups, (double2 *)ctx->d_stage);
+        err = cudaGetLastError();
+    }
+    if (err == cudaSuccess) err = cudaEventRecord(e1, ctx->stream);
+    if (err == cudaSuccess) err = cudaEventSynchronize(e1);
+    float ms = 0.f;
+    if (err == cudaSuccess) err = cudaEventElapsedTime(&ms, e0, e1);
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    if (err != cudaSuccess) return fail(ctx, QCD_ECUDA, "qcd_stream_bulk: %s", cudaGetErrorString(err));
     *ms_per_pass = (double)ms / reps;
     return QCD_OK;
 }

@@ -104,7 +104,7 @@ def test_guard_bands_dslash_families(q, dims, links, eps, prec):
         refs = ov.dslash_multi(dims, Uref, [_rounded(p, prec) for p in phis], -1)
         for n in (1, 2, 3, 4, 8):
             first = None
-            for kernel in ((0, 1, 2, 3) if n == 1 else (0, 4, 5, 6, 7, 8, 9)):
+            for kernel in ((0, 1, 2, 3) if n == 1 else (0, 4, 5, 6, 7, 8, 9, 10)):
                 ctx.qcd_set_dslash_variant(kernel)
                 for g in gout[:n]:
                     g.raw[GUARD: GUARD + g.n] = 0xFF                         # NaN: an element nobody writes stays NaN

@@ -421,6 +421,45 @@ def test_stream_read_hook(q, prec):
     ctx.close()
 
 
+def test_stream_bulk_hook(q):
+    """qcd_stream_bulk times the TMA path: tensor-map copies into a shared-memory ring, read back by consumer warps.  It must run for
+    every box shape the sweep of bench.py --stream-bulk uses (one producer warp and several, a ring of 2 and of 12 stages, boxes of 1,
+    3, 9 and 33 planes, a field smaller than one pass so that rows wrap), leave the field untouched, and reject bad arguments --
+    among them a stage ring that does not fit a block's shared memory, a lattice whose planes are not whole 128-site blocks, and a
+    precision-32 context."""
+    dims = (16, 16, 8, 4)                               # Vh = 4096 = 32 blocks of 128 sites
+    ctx = q.Context(dims, 64)
+    U = qcd_inputs.gauge_field(dims, "haar", seed=3)
+    fU = ctx.field(q.QCD_GAUGE).upload(U)
+    fe = ctx.field(q.QCD_SPINOR_EVEN).upload(qcd_inputs.gaussian_source(dims, seed=1, parity=0))
+    n0 = ctx.qcd_launch_count()
+    for rows, copies, stages, producers in ((9, 1, 4, 1), (3, 7, 4, 4), (33, 1, 3, 1), (1, 33, 3, 4), (3, 11, 2, 2), (1, 1, 12, 3)):
+        assert ctx.qcd_stream_bulk(fU, rows, copies, 8, stages, producers, 2) > 0.0
+    assert ctx.qcd_stream_bulk(fe, 3, 1, 5, 2, 1, 1) > 0.0                     # a three-plane field: every copy is the whole field's rows
+    assert ctx.qcd_launch_count() - n0 == 13
+    assert np.array_equal(fU.download(), U)
+    for bad in (lambda: ctx.qcd_stream_bulk(fU, 0, 1, 8, 3, 1, 1), lambda: ctx.qcd_stream_bulk(fU, 73, 1, 8, 2, 1, 1), lambda: ctx.qcd_stream_bulk(fe, 4, 1, 8, 2, 1, 1),
+                lambda: ctx.qcd_stream_bulk(fU, 9, 1, 8, 1, 1, 1), lambda: ctx.qcd_stream_bulk(fU, 9, 1, 8, 13, 1, 1), lambda: ctx.qcd_stream_bulk(fU, 9, 1, 8, 3, 5, 1),
+                lambda: ctx.qcd_stream_bulk(fU, 9, 1, 8, 3, 0, 1), lambda: ctx.qcd_stream_bulk(fU, 9, 1, 0, 3, 1, 1), lambda: ctx.qcd_stream_bulk(fU, 9, 1, 8, 3, 1, 0),
+                lambda: ctx.qcd_stream_bulk(fU, 33, 2, 8, 4, 1, 1)):                 # 4 x 66 x 2 KB of shared memory
+        with pytest.raises(q.QcdError):
+            bad()
+    ctx.close()
+    small = q.Context((4, 4, 4, 4), 64)                  # Vh = 128 is one block; (8,4,6,10): Vh = 960 is not a whole number of blocks
+    fs = small.field(q.QCD_GAUGE)
+    fs.buf.zero_()
+    assert small.qcd_stream_bulk(fs, 9, 1, 8, 2, 1, 1) > 0.0
+    small.close()
+    ragged = q.Context((8, 4, 6, 10), 64)
+    with pytest.raises(q.QcdError):
+        ragged.qcd_stream_bulk(ragged.field(q.QCD_GAUGE), 9, 1, 8, 2, 1, 1)
+    ragged.close()
+    c32 = q.Context(dims, 32)
+    with pytest.raises(q.QcdError):
+        c32.qcd_stream_bulk(c32.field(q.QCD_GAUGE), 9, 1, 8, 2, 1, 1)
+    c32.close()
+
+
 # ------------------------------------------------------------------------------------------
 # residual history: the recurrence, iteration by iteration, against the oracle's
 # ------------------------------------------------------------------------------------------

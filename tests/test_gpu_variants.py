@@ -252,7 +252,7 @@ def test_dslash_multi(q, n, prec, kind_name, tg):
         f.buf.zero_()
     refs = ov.dslash_multi(dims, Ur, [_rounded(p, prec) for p in phis], -1)
     first = None
-    for kernel in (0, 4, 5, 6, 7, 8, 9):  # library's choice; staged (links through shared memory); register kernel; pair kernel at two register caps; register kernel with the x0-x1 tile; rolled direction loop
+    for kernel in (0, 4, 5, 6, 7, 8, 9, 10):  # library's choice; staged (links through shared memory); register kernel; pair kernel at two register caps; register kernel with the x0-x1 tile; rolled direction loop; bulk-copy kernel (not applicable on this lattice: falls back)
         ctx.qcd_set_dslash_variant(kernel)
         for f in fout:
             f.buf.zero_()
@@ -266,6 +266,51 @@ def test_dslash_multi(q, n, prec, kind_name, tg):
             first = got
         else:                        # same FMAs in the same order per site, whichever way the operands arrive
             assert all(np.array_equal(a, b) for a, b in zip(first, got)), kernel
+    ctx.close()
+
+
+@pytest.mark.parametrize("prec", [64, 32])
+@pytest.mark.parametrize("dims,chunk", [((32, 8, 2, 4), 0), ((16, 16, 4, 2), 1), ((16, 16, 4, 2), 2), ((64, 4, 2, 2), 0), ((256, 2, 2, 2), 0),
+                                        ((128, 2, 4, 2), 0), ((32, 16, 4, 6), 0), ((16, 16, 16, 16), 0)])
+def test_dslash_bulk_copy_kernel_on_row_aligned_lattices(q, dims, chunk, prec):
+    """The warp-specialised bulk-copy kernel (variant 10; producer warps feed a shared-memory ring through the TMA engine, consumer
+    warps compute) needs a block's 128 sites to be whole x0-rows of one (x2, x3) plane.  Rows of 8 ... 128 sites (16, 8, 4, 2, 1 rows per
+    block), x1 wraps INSIDE a block (two runs per plane, the 1-d bulk copies) and at its edge, x2 / x3 extents of 2 (forward and backward
+    neighbour are the same site), with and without traversal chunking; every link storage (full, two-row, two-row in temporal gauge: unit
+    links are neither copied nor multiplied) and 2 ... 8 vectors (odd counts: one consumer half holds one vector fewer).
+    Bitwise equal to the register kernel, equal to the oracle within tolerance, and nothing is written outside the outputs."""
+    U = qcd_inputs.gauge_field(dims, "haar", seed=0)
+    Ufix, _ = ov.temporal_gauge(dims, U)
+    Ufix[qcd_inputs.site_coords(dims)[:, 3] != 0, 3] = np.eye(3)
+    par = qcd_inputs.site_parity(dims)
+    nmax = 8
+    ctx = q.Context(dims, prec, nrhs=nmax)
+    ctx.qcd_set_traversal_chunk(chunk)
+    phis = [qcd_inputs.gaussian_spinor(dims, seed=50 + i) for i in range(nmax)]
+    fin = [ctx.field(q.QCD_SPINOR_FULL).upload(p) for p in phis]
+    fout = [ctx.field(q.QCD_SPINOR_FULL) for _ in range(nmax)]
+    for name, kind, Uh, tg in (("full", q.QCD_GAUGE, U, False), ("tworow", q.QCD_GAUGE_2ROW, U, False), ("tworow+tg", q.QCD_GAUGE_2ROW, Ufix, True)):
+        fU = ctx.field(kind).upload(Uh)
+        ctx.qcd_gauge_set_temporal_unit(fU, tg)
+        Ur = _rounded(Uh, prec)
+        if kind == q.QCD_GAUGE_2ROW:
+            Ur = ov.reconstruct12(ov.compress12(Ur))
+        refs = ov.dslash_multi(dims, Ur, [_rounded(p, prec) for p in phis], -1)
+        for n in (2, 3, 5, 8):
+            res = {}
+            for kernel in (5, 10):
+                ctx.qcd_set_dslash_variant(kernel)
+                for f in fout:
+                    f.buf.fill_(255)
+                ctx.qcd_dslash_eo_multi(fU, fout[:n], fin[:n])
+                ctx.qcd_dslash_oe_multi(fU, fout[:n], fin[:n])
+                res[kernel] = [f.download() for f in fout[:n]]
+                assert all(bool((f.buf == 255).all().item()) for f in fout[n:]), (name, n, kernel)      # the other fields are untouched
+            for i in range(n):
+                for p in (0, 1):
+                    assert dslash_rel_err(res[10][i][par == p], refs[i][par == p]) <= DSLASH_TOL[prec], (name, n, i, p)
+            assert all(np.array_equal(a, b) for a, b in zip(res[5], res[10])), (name, n)
+    ctx.qcd_set_dslash_variant(0)
     ctx.close()
 
 
