@@ -22,7 +22,7 @@
 //       accumulate -- with the arithmetic of dslash_kernel, hop by hop in the same order, so the results are bitwise
 //       those of the other kernels.
 // What it reaches and what bounds it (profiles/r02_bulk_copy_kernel.md): fp64 full links at 64^4, n = 8: 3.41 - 3.67 ms against 3.55 - 3.57
-// of the register kernel, n = 6: 2.67 - 2.70 against 2.75 - 2.89; DRAM throughput 67 % against 57 % under ncu.  Every operand crosses shared
+// of the register kernel, n = 6: 2.67 - 2.70 against 2.75 - 2.89; DRAM throughput 66 % against 63 % under ncu.  Every operand crosses shared
 // memory twice (written by the copy engine, read by the consumers: 152 KB per hop and block at n = 8, 1190 cycles of the 128 B/cycle
 // crossbar), which together with the fp64 issue of eight consumer warps is where it stops: on a par, not ahead.  Slower for n <= 5,
 // for odd n (the two halves are unequal), on two-row links and in fp32.  Kept as variant 10 (qcd_set_dslash_variant), not dispatched.
