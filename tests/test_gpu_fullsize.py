@@ -163,6 +163,16 @@ def test_multi_vector_two_row_64(q, n):
             worst = max(worst, np.linalg.norm(got[lex(dims, x)] - ref) / max(np.linalg.norm(ref), 0.1 * R))
         assert worst <= DSLASH_TOL[64], (i, worst)
         del got
+    # the bulk-copy kernel (variant 10) at the same size, on the chunked traversal: bitwise the same fields, compared on the device
+    import torch
+    first = [f.buf.clone() for f in fout]
+    ctx.qcd_set_dslash_variant(10)
+    for f in fout:
+        f.buf.fill_(255)
+    ctx.qcd_dslash_oe_multi(f12, fout, fin)
+    torch.cuda.synchronize()
+    assert all(torch.equal(a, f.buf) for a, f in zip(first, fout))
+    ctx.qcd_set_dslash_variant(0)
     ctx.close()
 
 
