@@ -97,17 +97,22 @@ __device__ __forceinline__ unsigned long long global_ns()
 __device__ __forceinline__ double2 ld_coherent(const double2 *p) { return __ldcg(p); }
 __device__ __forceinline__ float2 ld_coherent(const float2 *p) { return __ldcg(p); }
 
-enum { PERSIST_BLOCK = 128, CLUSTER_MAX_CTAS = 16 };
+enum { CLUSTER_MAX_CTAS = 16 };
 // A lane keeps two links and up to four neighbour vectors in flight: 34 sixteen-byte loads = 136 registers in fp64.
 // Under a 168-register cap ptxas interleaves those loads with the FMAs that consume them (four dependent round trips
-// per phase instead of one), so the fp64 kernels run with a 255-register cap: 2 resident blocks of the grid version,
-// 256-thread CTAs in the cluster version (fp32: 4 blocks, 512 threads).
+// per phase instead of one), so the fp64 kernels run with a 255-register cap: ONE resident 256-thread block per SM in
+// the grid version (fp32: two, 128 registers), 128-thread CTAs in the cluster version (fp32: 512 threads).
+// Block shape of the grid version, measured per iteration (16^4 fp64 / fp32; 12^4; 16^3 x 32): 128 threads x 3 / x 4 resident
+// blocks 15.7 / 16.5, 11.0 / 12.3, 29.7 / 24.4 us; 256 x 1 / x 2: 14.5 / 15.3, 10.5 / 10.6, 24.6 / 25.3; 512 x 1: 14.9 / 16.4, -, 22.6 / 23.0;
+// fp32 1024 x 1: 17.0 at 16^4.  Half as many blocks arrive at every grid barrier and half as many partial sums are re-read
+// after it, and the fp64 lanes get their 255 registers; 256 is best at 16^4, the BASELINE.json config.
 // Measured (profiles/r02_small_lattice_timeline.md): the quad split halves the fp32 phases (3-5 us -> 1-2.6 us) and
 // is SLOWER in fp64 at every size (a lane's two links and four vectors are 136 registers of loads in flight; ptxas
 // interleaves them with the FMAs under a 168-register cap, and with a 255-register cap the index arithmetic, now
 // done by four lanes per site, fills the issue slots).  fp64 therefore keeps one thread per site (SPLIT = 1).
 template <typename T> struct PersistSplit { enum { value = sizeof(T) == 8 ? 1 : 4 }; };
-template <typename T> struct PersistMinB { enum { value = sizeof(T) == 8 ? 3 : 4 }; };
+template <typename T> struct PersistBlock { enum { value = 256 }; };
+template <typename T> struct PersistMinB { enum { value = sizeof(T) == 8 ? 1 : 2 }; };
 template <typename T> struct ClusterBlock { enum { value = sizeof(T) == 8 ? 128 : 512 }; };   // 16 CTAs hold 2048 sites either way
 
 // Barrier of the whole solve's thread set carrying this block's partial sum `block_val` (valid in thread 0; every
@@ -117,8 +122,10 @@ template <typename T> struct ClusterBlock { enum { value = sizeof(T) == 8 ? 128 
 //   CLUSTER: the solve is one thread-block cluster.  Thread 0 stores the partial into slot [epoch parity][own rank] of
 //            every CTA's shared memory, everybody meets at barrier.cluster, everybody adds the local slots in rank
 //            order.  The parity double-buffers the slots: a CTA cannot write epoch e + 2 before all have read e.
-//   grid   : cooperative launch; partials[block] then cooperative-groups grid.sync(), then every block re-reads all
-//            partials from the L2 and sums them thread-strided and through the block tree.
+//   grid   : cooperative launch; partials[epoch parity][block] then cooperative-groups grid.sync(), then every block re-reads
+//            all partials from the L2 and sums them thread-strided and through the block tree.  (A hand-written barrier on one
+//            monotonic arrival counter -- red.release + ld.acquire polling, no wait for the atomic's old value -- measured the
+//            same 1.8-2.6 us per barrier at 148 blocks: the cost is the drain of the block's stores, not the barrier's protocol.)
 template <int BLOCK, bool CLUSTER>
 __device__ __forceinline__ double solve_barrier(double block_val, unsigned epoch, double *partials, double *smem /* BLOCK/32 + 1 */,
                                                 double *cl_slots /* 2 x CLUSTER_MAX_CTAS, shared */)
@@ -136,6 +143,8 @@ __device__ __forceinline__ double solve_barrier(double block_val, unsigned epoch
         return s;
     } else {
         namespace cg = cooperative_groups;
+        partials += (size_t)(epoch & 1u) * gridDim.x;         // double-buffered like the cluster slots: a fast block may write its partial of
+                                                              // barrier e + 1 (phase 3 has no data barrier in front) while a slow one still sums barrier e
         if (threadIdx.x == 0) partials[blockIdx.x] = block_val;
         cg::this_grid().sync();
         double s = 0.0;
@@ -309,6 +318,9 @@ __device__ __forceinline__ void cg_persistent_body(const PersistArgs<T> &a)
     const int site0 = (int)blockIdx.x * spb;
     const int my_sites = Vh - site0 < spb ? (Vh - site0 > 0 ? Vh - site0 : 0) : spb;
     const int qpb = BLOCK / SPLIT, ql = (int)threadIdx.x / SPLIT, mu = (int)threadIdx.x % SPLIT;   // SPLIT = 1: one thread per site, mu = 0
+    // one trip: every thread (quad) has ONE site, the same in every phase -- then what phase 3 needs (p and Ap of the site from
+    // phase 2, x and r requested BEFORE the barrier that delivers alpha) is in registers when alpha arrives, Ap never goes to memory
+    const bool one_trip = spb <= qpb;
     unsigned epoch = 0;
     if (CLUSTER) cluster_barrier();                 // every CTA of the cluster is running before anyone stores into its shared memory
 
@@ -378,6 +390,7 @@ __device__ __forceinline__ void cg_persistent_body(const PersistArgs<T> &a)
         QCD_STAMP(2);
         // phase 2: Ap = m^2 p - D_eo t, partial Re<p,Ap>
         double dot = 0.0;
+        C kp[SPLIT == 1 ? 3 : 1], ka[SPLIT == 1 ? 3 : 1], kx[SPLIT == 1 ? 3 : 1], kr[SPLIT == 1 ? 3 : 1];   // one trip: p, Ap, x, r of this thread's site
         for (int o = 0; o < spb; o += qpb) {
             const int cb = site0 + o + ql;
             const bool active = o + ql < my_sites;
@@ -392,8 +405,13 @@ __device__ __forceinline__ void cg_persistent_body(const PersistArgs<T> &a)
                         C o;
                         o.x = fma(a.m2, vv[c].x, -acc[c].x);
                         o.y = fma(a.m2, vv[c].y, -acc[c].y);
-                        a.Ap[(size_t)c * sVh + cb] = o;
+                        if (one_trip) { kp[c] = vv[c]; ka[c] = o; }
+                        else a.Ap[(size_t)c * sVh + cb] = o;
                         dot += (double)vv[c].x * (double)o.x + (double)vv[c].y * (double)o.y;
+                    }
+                    if (one_trip) {
+#pragma unroll
+                        for (int c = 0; c < 3; ++c) { kx[c] = ld_coherent(a.x + (size_t)c * sVh + cb); kr[c] = ld_coherent(a.r + (size_t)c * sVh + cb); }
                     }
                 }
             } else {
@@ -409,7 +427,10 @@ __device__ __forceinline__ void cg_persistent_body(const PersistArgs<T> &a)
                     C o;
                     o.x = fma(a.m2, vv.x, -dc.x);
                     o.y = fma(a.m2, vv.y, -dc.y);
-                    a.Ap[(size_t)mu * sVh + cb] = o;
+                    if (one_trip) {
+                        kp[0] = vv; ka[0] = o;
+                        kx[0] = ld_coherent(a.x + (size_t)mu * sVh + cb); kr[0] = ld_coherent(a.r + (size_t)mu * sVh + cb);
+                    } else a.Ap[(size_t)mu * sVh + cb] = o;
                     dot += (double)vv.x * (double)o.x + (double)vv.y * (double)o.y;
                 }
             }
@@ -433,7 +454,8 @@ __device__ __forceinline__ void cg_persistent_body(const PersistArgs<T> &a)
 #pragma unroll
                     for (int c = 0; c < 3; ++c) {
                         const size_t i = (size_t)c * sVh + cb;
-                        vx[c] = ld_coherent(a.x + i); vr[c] = ld_coherent(a.r + i); vp[c] = ld_coherent(p_cur + i); va[c] = ld_coherent(a.Ap + i);
+                        if (one_trip) { vx[c] = kx[c]; vr[c] = kr[c]; vp[c] = kp[c]; va[c] = ka[c]; }
+                        else { vx[c] = ld_coherent(a.x + i); vr[c] = ld_coherent(a.r + i); vp[c] = ld_coherent(p_cur + i); va[c] = ld_coherent(a.Ap + i); }
                     }
 #pragma unroll
                     for (int c = 0; c < 3; ++c) {
@@ -445,8 +467,8 @@ __device__ __forceinline__ void cg_persistent_body(const PersistArgs<T> &a)
                     }
                 } else if (mu < 3) {                                // lane c of the quad: colour c of the site
                     const size_t i = (size_t)mu * sVh + cb;
-                    C vx = ld_coherent(a.x + i), vr = ld_coherent(a.r + i);
-                    const C vp = ld_coherent(p_cur + i), va = ld_coherent(a.Ap + i);
+                    C vx = one_trip ? kx[0] : ld_coherent(a.x + i), vr = one_trip ? kr[0] : ld_coherent(a.r + i);
+                    const C vp = one_trip ? kp[0] : ld_coherent(p_cur + i), va = one_trip ? ka[0] : ld_coherent(a.Ap + i);
                     vx.x = fma(al, vp.x, vx.x); vx.y = fma(al, vp.y, vx.y);
                     vr.x = fma(-al, va.x, vr.x); vr.y = fma(-al, va.y, vr.y);
                     a.x[i] = vx; a.r[i] = vr;
@@ -484,9 +506,9 @@ __device__ __forceinline__ void cg_persistent_body(const PersistArgs<T> &a)
 
 // cooperative launch, any number of co-resident blocks
 template <typename T, int NROW, int TG>
-__global__ void __launch_bounds__(PERSIST_BLOCK, PersistMinB<T>::value) cg_persistent_kernel(const PersistArgs<T> a)
+__global__ void __launch_bounds__(PersistBlock<T>::value, PersistMinB<T>::value) cg_persistent_kernel(const PersistArgs<T> a)
 {
-    cg_persistent_body<T, NROW, TG, PERSIST_BLOCK, false, PersistSplit<T>::value>(a);
+    cg_persistent_body<T, NROW, TG, PersistBlock<T>::value, false, PersistSplit<T>::value>(a);
 }
 
 // ONE cluster of 1 .. 16 CTAs (cluster dimension = grid dimension, set at launch)

@@ -1045,6 +1045,7 @@ static qcd_status cg_persistent_launch(qcd_ctx *c, bool probe_only, bool *ok)
     }
 
     auto kernel = cg_persistent_kernel<T, NROW, TG>;
+    enum { PERSIST_BLOCK = PersistBlock<T>::value };
     int per_sm = 0, sms = 0, coop = 0;
     CU(c, cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, c->dev));
     CU(c, cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, c->dev));
@@ -1052,10 +1053,10 @@ static qcd_status cg_persistent_launch(qcd_ctx *c, bool probe_only, bool *ok)
     *ok = coop && per_sm > 0;
     if (probe_only || !*ok) return QCD_OK;
     // Every block owns an equally long range of sites (cg_persistent.cuh): launch k blocks on EVERY SM, k the smallest number
-    // of co-resident blocks that covers the sites in one pass (16^4 fp64: 2 x 148 blocks of 112 sites), capped by what is
+    // of co-resident blocks that covers the sites in one pass (16^4 fp64: 148 blocks of 256 threads, 222 sites each), capped by what is
     // co-resident (then a block walks its range in several trips); tiny lattices get one block per warp of work.
     int max_grid = per_sm * sms;
-    if (max_grid * MAXRHS > c->partials_cap) max_grid = c->partials_cap / MAXRHS;
+    if (max_grid * 2 > c->partials_cap) max_grid = c->partials_cap / 2;       // two buffers of per-block partials (solve_barrier)
     int k = (wanted_threads + sms * PERSIST_BLOCK - 1) / (sms * PERSIST_BLOCK);
     if (k > per_sm) k = per_sm;
     int grid = sms * k;
