@@ -309,8 +309,8 @@ __device__ __forceinline__ void cg_persistent_body(const PersistArgs<T> &a)
     const size_t sVh = (size_t)Vh;
     const int gtid = blockIdx.x * BLOCK + threadIdx.x;
     // Every block owns one contiguous range of sites (the same in every phase and iteration, so phase 3 updates what the
-    // same SM wrote in phase 2), all ranges equally long; the host launches a multiple of the SM count (16^4 fp64: 2 x 148
-    // blocks of 112 sites instead of 256 blocks of 128 sites on 148 SMs); the range length is even so that a block starts
+    // same SM wrote in phase 2), all ranges equally long; the host launches a multiple of the SM count (16^4 fp64: 148
+    // blocks of 222 sites instead of 256 blocks of 128 sites on 148 SMs); the range length is even so that a block starts
     // on a 32-byte sector.  Measured: no change at 16^4 (15.9 us either way -- the phases run at 80 % of the aggregate
     // L2 stream, not at a per-SM limit), kept because every SM now carries the same load at every lattice size.
     int spb = (Vh + (int)gridDim.x - 1) / (int)gridDim.x;
