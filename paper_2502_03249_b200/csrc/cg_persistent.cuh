@@ -22,18 +22,17 @@
 //
 // What the phase timeline showed (qcd_cg_timeline_*, profiles/r02_small_lattice_timeline.md) and what this
 // file does about it:
-//   * up to 12^4 a phase is a chain of L2 round trips (~0.3 us each), not bandwidth: with one thread per
-//     site the 168-register cap makes ptxas walk the four directions one after the other (2.2 us per
-//     Dslash phase at 4^4 ... 12^4 alike).  A site is therefore handled by a QUAD of lanes, one direction
-//     each: every lane issues all the loads of its forward and backward hop at once (one round trip), the
-//     four partial sums meet in two shuffle steps, and lanes 0..2 of the quad finish one colour each;
+//   * up to 12^4 a phase is a chain of L2 round trips (~0.3 us each), not bandwidth: under a 168-register cap ptxas walks
+//     the four directions one after the other (2.2 us per Dslash phase at 4^4 ... 12^4 alike).  A thread therefore gets the
+//     whole register file's share of ONE 256-thread block per SM (255 registers: all loads of a site in flight at once); an
+//     earlier version split a site over a quad of lanes instead, which the wider cap made unnecessary (see PersistBlock);
 //   * a cooperative-groups grid.sync() costs 1.2-1.8 us and the re-read of the per-block partials after it
 //     another 0.4-0.9 us: 6 of the 15.8 us of a 16^4 iteration and of the 11 us of an 8^4 one.  Two hand-written
 //     replacements (every block polling every block's tagged slot, by all threads and by one warp with a 128-byte
 //     line per slot) were SLOWER from 4 blocks on (2.7 us at 4 blocks, 4-5 us at 64, 7-10 us at 340: the polls
 //     of an all-gather grow with the square of the grid) and grid.sync() stays for grids of several clusters.
-//     Lattices of up to 2048 sites per parity (8^4) run as ONE thread-block cluster of up to 16 CTAs x 512
-//     threads (fp64: 256) instead: the barrier is the hardware barrier.cluster (release / acquire at cluster scope), and the
+//     Lattices of up to 2048 sites per parity (8^4) run as ONE thread-block cluster of up to 16 CTAs x 128
+//     threads instead: the barrier is the hardware barrier.cluster (release / acquire at cluster scope), and the
 //     partial sums are exchanged through distributed shared memory -- every CTA stores its partial into every
 //     peer's slot before it arrives and sums the 16 local slots in rank order after the wait.
 //
@@ -98,22 +97,21 @@ __device__ __forceinline__ double2 ld_coherent(const double2 *p) { return __ldcg
 __device__ __forceinline__ float2 ld_coherent(const float2 *p) { return __ldcg(p); }
 
 enum { CLUSTER_MAX_CTAS = 16 };
-// A lane keeps two links and up to four neighbour vectors in flight: 34 sixteen-byte loads = 136 registers in fp64.
-// Under a 168-register cap ptxas interleaves those loads with the FMAs that consume them (four dependent round trips
-// per phase instead of one), so the fp64 kernels run with a 255-register cap: ONE resident 256-thread block per SM in
-// the grid version (fp32: two, 128 registers), 128-thread CTAs in the cluster version (fp32: 512 threads).
+// One thread per site, in both precisions.  A thread keeps two links and up to four neighbour vectors in flight: 34 sixteen-byte loads
+// = 136 registers in fp64.  Under a 168-register cap ptxas interleaves those loads with the FMAs that consume them (four dependent round
+// trips per phase instead of one), so the kernels run with a 255-register cap: ONE resident 256-thread block per SM in the grid
+// version, 128-thread CTAs in the cluster version.
 // Block shape of the grid version, measured per iteration (16^4 fp64 / fp32; 12^4; 16^3 x 32): 128 threads x 3 / x 4 resident
-// blocks 15.7 / 16.5, 11.0 / 12.3, 29.7 / 24.4 us; 256 x 1 / x 2: 14.5 / 15.3, 10.5 / 10.6, 24.6 / 25.3; 512 x 1: 14.9 / 16.4, -, 22.6 / 23.0;
-// fp32 1024 x 1: 17.0 at 16^4.  Half as many blocks arrive at every grid barrier and half as many partial sums are re-read
-// after it, and the fp64 lanes get their 255 registers; 256 is best at 16^4, the BASELINE.json config.
-// Measured (profiles/r02_small_lattice_timeline.md): the quad split halves the fp32 phases (3-5 us -> 1-2.6 us) and
-// is SLOWER in fp64 at every size (a lane's two links and four vectors are 136 registers of loads in flight; ptxas
-// interleaves them with the FMAs under a 168-register cap, and with a 255-register cap the index arithmetic, now
-// done by four lanes per site, fills the issue slots).  fp64 therefore keeps one thread per site (SPLIT = 1).
-template <typename T> struct PersistSplit { enum { value = sizeof(T) == 8 ? 1 : 4 }; };
+// blocks 15.7 / 16.5, 11.0 / 12.3, 29.7 / 24.4 us; 256 x 1 / x 2: 14.5 / 15.3, 10.5 / 10.6, 24.6 / 25.3; 512 x 1: 14.9 / 16.4, -, 22.6 / 23.0.
+// Half as many blocks arrive at every grid barrier and half as many partial sums are re-read after it, and a thread gets its 255
+// registers; 256 is best at 16^4, the BASELINE.json config.
+// History (profiles/r02_small_lattice_timeline.md): under the earlier 128-register cap the fp32 kernel split a site over a QUAD of
+// lanes, one direction each (phases 3-5 us -> 1-2.6 us).  With one 256-thread block per SM and 255 registers the plain form is the
+// faster one in fp32 as well -- 16^4 15.1 -> 11.3 us per iteration, 16^3 x 32 25.4 -> 17.1, 8^4 8.5 -> 7.1, 4^4 7.6 -> 6.9 -- and the quad
+// path is gone (in fp64 it had been slower at every size).
 template <typename T> struct PersistBlock { enum { value = 256 }; };
-template <typename T> struct PersistMinB { enum { value = sizeof(T) == 8 ? 1 : 2 }; };
-template <typename T> struct ClusterBlock { enum { value = sizeof(T) == 8 ? 128 : 512 }; };   // 16 CTAs hold 2048 sites either way
+template <typename T> struct PersistMinB { enum { value = 1 }; };
+template <typename T> struct ClusterBlock { enum { value = 128 }; };   // 16 CTAs hold 2048 sites
 
 // Barrier of the whole solve's thread set carrying this block's partial sum `block_val` (valid in thread 0; every
 // thread of the block has passed a __syncthreads() after its last global store of the phase -- block_sum provides
@@ -205,103 +203,9 @@ __device__ __forceinline__ void persistent_site(typename Cplx<T>::type acc[3], c
     }
 }
 
-// One direction (forward and backward hop) of (D in)(cb) for the site cb of `parity`: lane mu of a quad.
-// FUSE: the input vector is r + beta * in, formed at both neighbours on the fly.  All loads are issued before
-// the first use.  Same helpers and the same FMA order per hop as dslash_kernel; the four directions are then
-// added as (d0 + d1) + (d2 + d3) by quad_sum (dslash_kernel adds them one after the other).
-template <typename T, int NROW, int TG, bool FUSE, bool KEEP_L1>
-__device__ __forceinline__ void persistent_dir(typename Cplx<T>::type acc[3], const Lattice &L, int parity, int cb, int mu,
-                                               const typename Cplx<T>::type *U, const typename Cplx<T>::type *in,
-                                               const typename Cplx<T>::type *r, T beta)
-{
-    typedef typename Cplx<T>::type C;
-    const size_t Vh = (size_t)L.Vh;
-    const unsigned ucb = (unsigned)cb;
-    const int xh = (int)(ucb % (unsigned)L.h);
-    unsigned q = ucb / (unsigned)L.h;
-    const int x1 = (int)(q % (unsigned)L.N1);
-    q /= (unsigned)L.N1;
-    const int x2 = (int)(q % (unsigned)L.N2);
-    const int x3 = (int)(q / (unsigned)L.N2);
-    const int rp = (x1 + x2 + x3 + parity) & 1;           // x0 = 2 xh + rp
-    int nf, nb;
-    if (mu == 0) {
-        nf = rp ? ((xh + 1 == L.h) ? cb - (L.h - 1) : cb + 1) : cb;
-        nb = rp ? cb : ((xh == 0) ? cb + (L.h - 1) : cb - 1);
-    } else {
-        const int xm = mu == 1 ? x1 : (mu == 2 ? x2 : x3);
-        const int Nm = mu == 1 ? L.N1 : (mu == 2 ? L.N2 : L.N3);
-        const int sm = mu == 1 ? L.s1 : (mu == 2 ? L.s2 : L.s3);
-        nf = (xm + 1 == Nm) ? cb - (Nm - 1) * sm : cb + sm;
-        nb = (xm == 0) ? cb + (Nm - 1) * sm : cb - sm;
-    }
-    // eta_mu(x) = (-1)^{x0 + ... + x_{mu-1}}; the forward term carries eta (times -1 across the time seam), the backward
-    // term MINUS eta (R3, R4)
-    const unsigned e = (unsigned)((mu >= 1 ? rp : 0) + (mu >= 2 ? x1 : 0) + (mu >= 3 ? x2 : 0)) & 1u;
-    const unsigned negf = e ^ ((mu == 3 && x3 + 1 == L.N3) ? 1u : 0u);
-    const unsigned negb = (e ^ 1u) ^ ((mu == 3 && x3 == 0) ? 1u : 0u);
-    const bool unit_f = TG && mu == 3 && x3 != 0;
-    const bool unit_b = TG && mu == 3 && x3 != 1;
-
-    const uint64_t pol = l2_policy_evict_last();             // everything is meant to stay in the L2 here
-    const C *Uf = U + (size_t)(parity * 12 * NROW + mu * 3 * NROW) * Vh + cb;
-    const C *Ub = U + (size_t)((1 - parity) * 12 * NROW + mu * 3 * NROW) * Vh + nb;
-    C uf[9], ub[9], pf[3], pb[3], rf[3], rb[3];
-    // KEEP_L1 (one-cluster solves): a CTA handles the same sites in every iteration, so its links may stay in its L1
-    if (!unit_f) {
-#pragma unroll
-        for (int k = 0; k < 3 * NROW; ++k) uf[k] = KEEP_L1 ? ld_keep(Uf + (size_t)k * Vh, pol) : ld_stream(Uf + (size_t)k * Vh, pol);
-    }
-    if (!unit_b) {
-#pragma unroll
-        for (int k = 0; k < 3 * NROW; ++k) ub[k] = KEEP_L1 ? ld_keep(Ub + (size_t)k * Vh, pol) : ld_stream(Ub + (size_t)k * Vh, pol);
-    }
-#pragma unroll
-    for (int c = 0; c < 3; ++c) {
-        pf[c] = ld_coherent(in + (size_t)c * Vh + nf);
-        pb[c] = ld_coherent(in + (size_t)c * Vh + nb);
-        if (FUSE) { rf[c] = ld_coherent(r + (size_t)c * Vh + nf); rb[c] = ld_coherent(r + (size_t)c * Vh + nb); }
-    }
-#pragma unroll
-    for (int c = 0; c < 3; ++c) {
-        if (FUSE) {
-            pf[c].x = fma(beta, pf[c].x, rf[c].x); pf[c].y = fma(beta, pf[c].y, rf[c].y);
-            pb[c].x = fma(beta, pb[c].x, rb[c].x); pb[c].y = fma(beta, pb[c].y, rb[c].y);
-        }
-        pf[c].x = flip_sign(pf[c].x, negf); pf[c].y = flip_sign(pf[c].y, negf);
-        pb[c].x = flip_sign(pb[c].x, negb); pb[c].y = flip_sign(pb[c].y, negb);
-    }
-    if (!unit_f) { if (NROW == 2) reconstruct_third_row<C>(uf); mat_vec_acc<T, C>(acc, uf, pf); } else vec_acc<C>(acc, pf);
-    if (!unit_b) { if (NROW == 2) reconstruct_third_row<C>(ub); matdag_vec_acc<T, C>(acc, ub, pb); } else vec_acc<C>(acc, pb);
-}
-
-// sum over the four lanes of a quad, (l0 + l1) + (l2 + l3); every lane ends with the same bits (fp addition commutes)
-__device__ __forceinline__ double quad_add(double v)
-{
-    v += __shfl_xor_sync(0xffffffffu, v, 1);
-    v += __shfl_xor_sync(0xffffffffu, v, 2);
-    return v;
-}
-__device__ __forceinline__ float quad_add(float v)
-{
-    v += __shfl_xor_sync(0xffffffffu, v, 1);
-    v += __shfl_xor_sync(0xffffffffu, v, 2);
-    return v;
-}
-template <typename C>
-__device__ __forceinline__ C quad_sum_pick(const C acc[3], int lane_in_quad)
-{
-    C a0, a1, a2;
-    a0.x = quad_add(acc[0].x); a0.y = quad_add(acc[0].y);
-    a1.x = quad_add(acc[1].x); a1.y = quad_add(acc[1].y);
-    a2.x = quad_add(acc[2].x); a2.y = quad_add(acc[2].y);
-    return lane_in_quad == 0 ? a0 : (lane_in_quad == 1 ? a1 : a2);     // lane c < 3 finishes colour c
-}
-
-template <typename T, int NROW, int TG, int BLOCK, bool CLUSTER, int SPLIT>
+template <typename T, int NROW, int TG, int BLOCK, bool CLUSTER>
 __device__ __forceinline__ void cg_persistent_body(const PersistArgs<T> &a)
 {
-    static_assert(SPLIT == 1 || SPLIT == 4, "a site is one thread or a quad of lanes");
     typedef typename Cplx<T>::type C;
     __shared__ double smem[BLOCK / 32 + 1];
     __shared__ double cl_slots[2 * CLUSTER_MAX_CTAS];
@@ -317,8 +221,8 @@ __device__ __forceinline__ void cg_persistent_body(const PersistArgs<T> &a)
     spb += spb & 1;
     const int site0 = (int)blockIdx.x * spb;
     const int my_sites = Vh - site0 < spb ? (Vh - site0 > 0 ? Vh - site0 : 0) : spb;
-    const int qpb = BLOCK / SPLIT, ql = (int)threadIdx.x / SPLIT, mu = (int)threadIdx.x % SPLIT;   // SPLIT = 1: one thread per site, mu = 0
-    // one trip: every thread (quad) has ONE site, the same in every phase -- then what phase 3 needs (p and Ap of the site from
+    const int qpb = BLOCK, ql = (int)threadIdx.x;               // one thread per site: sites per trip of a block, this thread's site in the trip
+    // one trip: every thread has ONE site, the same in every phase -- then what phase 3 needs (p and Ap of the site from
     // phase 2, x and r requested BEFORE the barrier that delivers alpha) is in registers when alpha arrives, Ap never goes to memory
     const bool one_trip = spb <= qpb;
     unsigned epoch = 0;
@@ -343,10 +247,10 @@ __device__ __forceinline__ void cg_persistent_body(const PersistArgs<T> &a)
         QCD_STAMP(0);
         // phase 1: p_cur = r + beta p_old (own even site), t = D_oe p_cur (formed on the fly at the neighbours)
         const T be = (T)beta;
-        for (int o = 0; o < spb; o += qpb) {                     // the same trip count in every thread: the quad shuffles are warp-wide
+        for (int o = 0; o < spb; o += qpb) {                     // the same trip count in every thread
             const int cb = site0 + o + ql;
             const bool active = o + ql < my_sites;
-            if (SPLIT == 1) {
+            {
                 if (active) {
                     C acc[3];
                     persistent_site<T, NROW, TG, true, CLUSTER>(acc, a.L, 1, cb, a.U, p_old, a.r, be);
@@ -365,23 +269,6 @@ __device__ __forceinline__ void cg_persistent_body(const PersistArgs<T> &a)
                         p_cur[(size_t)c * sVh + cb] = vp[c];
                     }
                 }
-            } else {
-                C acc[3], vp, vr;
-                acc[0].x = acc[0].y = acc[1].x = acc[1].y = acc[2].x = acc[2].y = (T)0;
-                vp.x = vp.y = vr.x = vr.y = (T)0;
-                if (active) {
-                    if (mu < 3) {                                // the site-local operands travel with the neighbour loads
-                        vp = ld_coherent(p_old + (size_t)mu * sVh + cb);
-                        vr = ld_coherent(a.r + (size_t)mu * sVh + cb);
-                    }
-                    persistent_dir<T, NROW, TG, true, CLUSTER>(acc, a.L, 1, cb, mu, a.U, p_old, a.r, be);
-                }
-                const C tc = quad_sum_pick<C>(acc, mu);
-                if (active && mu < 3) {
-                    a.t[(size_t)mu * sVh + cb] = tc;
-                    vp.x = fma(be, vp.x, vr.x); vp.y = fma(be, vp.y, vr.y);
-                    p_cur[(size_t)mu * sVh + cb] = vp;
-                }
             }
         }
         QCD_STAMP(1);
@@ -390,11 +277,11 @@ __device__ __forceinline__ void cg_persistent_body(const PersistArgs<T> &a)
         QCD_STAMP(2);
         // phase 2: Ap = m^2 p - D_eo t, partial Re<p,Ap>
         double dot = 0.0;
-        C kp[SPLIT == 1 ? 3 : 1], ka[SPLIT == 1 ? 3 : 1], kx[SPLIT == 1 ? 3 : 1], kr[SPLIT == 1 ? 3 : 1];   // one trip: p, Ap, x, r of this thread's site
+        C kp[3], ka[3], kx[3], kr[3];                             // one trip: p, Ap, x, r of this thread's site
         for (int o = 0; o < spb; o += qpb) {
             const int cb = site0 + o + ql;
             const bool active = o + ql < my_sites;
-            if (SPLIT == 1) {
+            {
                 if (active) {
                     C acc[3], vv[3];
                     persistent_site<T, NROW, TG, false, CLUSTER>(acc, a.L, 0, cb, a.U, a.t);
@@ -414,25 +301,6 @@ __device__ __forceinline__ void cg_persistent_body(const PersistArgs<T> &a)
                         for (int c = 0; c < 3; ++c) { kx[c] = ld_coherent(a.x + (size_t)c * sVh + cb); kr[c] = ld_coherent(a.r + (size_t)c * sVh + cb); }
                     }
                 }
-            } else {
-                C acc[3], vv;
-                acc[0].x = acc[0].y = acc[1].x = acc[1].y = acc[2].x = acc[2].y = (T)0;
-                vv.x = vv.y = (T)0;
-                if (active) {
-                    if (mu < 3) vv = ld_coherent(p_cur + (size_t)mu * sVh + cb);
-                    persistent_dir<T, NROW, TG, false, CLUSTER>(acc, a.L, 0, cb, mu, a.U, a.t, nullptr, (T)0);
-                }
-                const C dc = quad_sum_pick<C>(acc, mu);
-                if (active && mu < 3) {
-                    C o;
-                    o.x = fma(a.m2, vv.x, -dc.x);
-                    o.y = fma(a.m2, vv.y, -dc.y);
-                    if (one_trip) {
-                        kp[0] = vv; ka[0] = o;
-                        kx[0] = ld_coherent(a.x + (size_t)mu * sVh + cb); kr[0] = ld_coherent(a.r + (size_t)mu * sVh + cb);
-                    } else a.Ap[(size_t)mu * sVh + cb] = o;
-                    dot += (double)vv.x * (double)o.x + (double)vv.y * (double)o.y;
-                }
             }
         }
         const double dot_block = block_sum<BLOCK>(dot, smem);
@@ -449,7 +317,7 @@ __device__ __forceinline__ void cg_persistent_body(const PersistArgs<T> &a)
         for (int o = 0; o < spb; o += qpb) {
             const int cb = site0 + o + ql;
             if (o + ql < my_sites) {
-                if (SPLIT == 1) {
+                {
                     C vx[3], vr[3], vp[3], va[3];
 #pragma unroll
                     for (int c = 0; c < 3; ++c) {
@@ -465,14 +333,6 @@ __device__ __forceinline__ void cg_persistent_body(const PersistArgs<T> &a)
                         a.x[i] = vx[c]; a.r[i] = vr[c];
                         nrm += (double)vr[c].x * (double)vr[c].x + (double)vr[c].y * (double)vr[c].y;
                     }
-                } else if (mu < 3) {                                // lane c of the quad: colour c of the site
-                    const size_t i = (size_t)mu * sVh + cb;
-                    C vx = one_trip ? kx[0] : ld_coherent(a.x + i), vr = one_trip ? kr[0] : ld_coherent(a.r + i);
-                    const C vp = one_trip ? kp[0] : ld_coherent(p_cur + i), va = one_trip ? ka[0] : ld_coherent(a.Ap + i);
-                    vx.x = fma(al, vp.x, vx.x); vx.y = fma(al, vp.y, vx.y);
-                    vr.x = fma(-al, va.x, vr.x); vr.y = fma(-al, va.y, vr.y);
-                    a.x[i] = vx; a.r[i] = vr;
-                    nrm += (double)vr.x * (double)vr.x + (double)vr.y * (double)vr.y;
                 }
             }
         }
@@ -508,14 +368,14 @@ __device__ __forceinline__ void cg_persistent_body(const PersistArgs<T> &a)
 template <typename T, int NROW, int TG>
 __global__ void __launch_bounds__(PersistBlock<T>::value, PersistMinB<T>::value) cg_persistent_kernel(const PersistArgs<T> a)
 {
-    cg_persistent_body<T, NROW, TG, PersistBlock<T>::value, false, PersistSplit<T>::value>(a);
+    cg_persistent_body<T, NROW, TG, PersistBlock<T>::value, false>(a);
 }
 
 // ONE cluster of 1 .. 16 CTAs (cluster dimension = grid dimension, set at launch)
 template <typename T, int NROW, int TG>
 __global__ void __launch_bounds__(ClusterBlock<T>::value, 1) cg_cluster_kernel(const PersistArgs<T> a)
 {
-    cg_persistent_body<T, NROW, TG, ClusterBlock<T>::value, true, PersistSplit<T>::value>(a);
+    cg_persistent_body<T, NROW, TG, ClusterBlock<T>::value, true>(a);
 }
 
 } // namespace qcd

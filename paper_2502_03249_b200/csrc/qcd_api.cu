@@ -1012,8 +1012,7 @@ static qcd_status cg_persistent_launch(qcd_ctx *c, bool probe_only, bool *ok)
     a.p2 = (C *)ws_at(c, 4, 1, 0);
     a.m2 = (T)(c->cg.m * c->cg.m); a.partials = c->d_partials; a.scal = c->d_scal;
     a.timeline = c->timeline_on ? c->d_timeline : nullptr;
-    enum { SPLIT = PersistSplit<T>::value };                     // lanes per site (cg_persistent.cuh)
-    const int wanted_threads = SPLIT * c->L.Vh;
+    const int wanted_threads = c->L.Vh;                         // one thread per site (cg_persistent.cuh)
 
     // up to 2048 sites per parity: ONE thread-block cluster (hardware barrier, partial sums through DSMEM)
     enum { CLUSTER_BLOCK = ClusterBlock<T>::value };
