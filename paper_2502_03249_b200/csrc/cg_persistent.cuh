@@ -34,7 +34,9 @@
 //     Lattices of up to 2048 sites per parity (8^4) run as ONE thread-block cluster of up to 16 CTAs x 128
 //     threads instead: the barrier is the hardware barrier.cluster (release / acquire at cluster scope), and the
 //     partial sums are exchanged through distributed shared memory -- every CTA stores its partial into every
-//     peer's slot before it arrives and sums the 16 local slots in rank order after the wait.
+//     peer's slot before it arrives and sums the 16 local slots in rank order after the wait.  In that shape the
+//     vectors the neighbours read (r, both direction buffers, t) live in the CTAs' shared memory as well and are
+//     gathered with ld.shared::cluster, x and Ap stay in registers for the whole solve (cg_cluster_body below).
 //
 // Fields written inside the kernel (p, t, Ap, r, x) are read with L2-coherent loads (ld.global.cg),
 // never through the read-only path; links are read-only and keep it.
@@ -66,6 +68,26 @@ __device__ __forceinline__ void st_shared_cluster(double *local, unsigned rank, 
     unsigned ra;
     asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(ra) : "r"(la), "r"(rank));
     asm volatile("st.shared::cluster.f64 [%0], %1;" :: "r"(ra), "d"(v) : "memory");
+}
+
+// load a complex number from the shared memory of CTA `rank` of the cluster, at the address that `local` has in this CTA
+__device__ __forceinline__ double2 ld_shared_cluster(const double2 *local, unsigned rank)
+{
+    const unsigned la = (unsigned)__cvta_generic_to_shared(local);
+    unsigned ra;
+    double2 v;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(ra) : "r"(la), "r"(rank));
+    asm volatile("ld.shared::cluster.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "r"(ra) : "memory");
+    return v;
+}
+__device__ __forceinline__ float2 ld_shared_cluster(const float2 *local, unsigned rank)
+{
+    const unsigned la = (unsigned)__cvta_generic_to_shared(local);
+    unsigned ra;
+    float2 v;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(ra) : "r"(la), "r"(rank));
+    asm volatile("ld.shared::cluster.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "r"(ra) : "memory");
+    return v;
 }
 
 template <typename T>
@@ -203,12 +225,13 @@ __device__ __forceinline__ void persistent_site(typename Cplx<T>::type acc[3], c
     }
 }
 
-template <typename T, int NROW, int TG, int BLOCK, bool CLUSTER>
+// The grid version (cooperative launch): vectors in global memory, read through the L2.
+template <typename T, int NROW, int TG, int BLOCK>
 __device__ __forceinline__ void cg_persistent_body(const PersistArgs<T> &a)
 {
     typedef typename Cplx<T>::type C;
     __shared__ double smem[BLOCK / 32 + 1];
-    __shared__ double cl_slots[2 * CLUSTER_MAX_CTAS];
+    double *const cl_slots = nullptr;                           // (cluster version only)
     const int Vh = a.L.Vh;
     const size_t sVh = (size_t)Vh;
     const int gtid = blockIdx.x * BLOCK + threadIdx.x;
@@ -226,7 +249,6 @@ __device__ __forceinline__ void cg_persistent_body(const PersistArgs<T> &a)
     // phase 2, x and r requested BEFORE the barrier that delivers alpha) is in registers when alpha arrives, Ap never goes to memory
     const bool one_trip = spb <= qpb;
     unsigned epoch = 0;
-    if (CLUSTER) cluster_barrier();                 // every CTA of the cluster is running before anyone stores into its shared memory
 
     // the recurrence state, replicated: every thread of every block holds the same values
     double rr = a.scal->rr;
@@ -253,7 +275,7 @@ __device__ __forceinline__ void cg_persistent_body(const PersistArgs<T> &a)
             {
                 if (active) {
                     C acc[3];
-                    persistent_site<T, NROW, TG, true, CLUSTER>(acc, a.L, 1, cb, a.U, p_old, a.r, be);
+                    persistent_site<T, NROW, TG, true, false>(acc, a.L, 1, cb, a.U, p_old, a.r, be);
                     // all six loads before the first store: one L2 round trip instead of three (a load issued after a
                     // store that may alias it waits for that store)
                     C vp[3], vr[3];
@@ -272,8 +294,7 @@ __device__ __forceinline__ void cg_persistent_body(const PersistArgs<T> &a)
             }
         }
         QCD_STAMP(1);
-        if (CLUSTER) cluster_barrier();                          // data barrier: t and p_cur are complete everywhere
-        else cooperative_groups::this_grid().sync();
+        cooperative_groups::this_grid().sync();                  // data barrier: t and p_cur are complete everywhere
         QCD_STAMP(2);
         // phase 2: Ap = m^2 p - D_eo t, partial Re<p,Ap>
         double dot = 0.0;
@@ -284,7 +305,7 @@ __device__ __forceinline__ void cg_persistent_body(const PersistArgs<T> &a)
             {
                 if (active) {
                     C acc[3], vv[3];
-                    persistent_site<T, NROW, TG, false, CLUSTER>(acc, a.L, 0, cb, a.U, a.t);
+                    persistent_site<T, NROW, TG, false, false>(acc, a.L, 0, cb, a.U, a.t);
 #pragma unroll
                     for (int c = 0; c < 3; ++c) vv[c] = ld_coherent(p_cur + (size_t)c * sVh + cb);
 #pragma unroll
@@ -305,7 +326,7 @@ __device__ __forceinline__ void cg_persistent_body(const PersistArgs<T> &a)
         }
         const double dot_block = block_sum<BLOCK>(dot, smem);
         QCD_STAMP(3);
-        pAp = solve_barrier<BLOCK, CLUSTER>(dot_block, ++epoch, a.partials, smem, cl_slots);
+        pAp = solve_barrier<BLOCK, false>(dot_block, ++epoch, a.partials, smem, cl_slots);
         QCD_STAMP(4);
         if (!(pAp > 0.0)) { flag = 3; break; }                     // breakdown: uniform across the grid
         alpha = rr / pAp;
@@ -339,7 +360,7 @@ __device__ __forceinline__ void cg_persistent_body(const PersistArgs<T> &a)
         __syncthreads();                                           // smem of the previous barrier has been read by everyone
         const double nrm_block = block_sum<BLOCK>(nrm, smem);
         QCD_STAMP(6);
-        const double rr_new = solve_barrier<BLOCK, CLUSTER>(nrm_block, ++epoch, a.partials, smem, cl_slots);
+        const double rr_new = solve_barrier<BLOCK, false>(nrm_block, ++epoch, a.partials, smem, cl_slots);
         QCD_STAMP(7);
         beta = rr_new / rr;
         rr = rr_new;
@@ -361,21 +382,243 @@ __device__ __forceinline__ void cg_persistent_body(const PersistArgs<T> &a)
         CgScalars *s = a.scal;
         s->rr = rr; s->pAp = pAp; s->alpha = alpha; s->beta = beta; s->k = k; s->flag = flag;
     }
-    if (CLUSTER) cluster_barrier();                 // no CTA exits while a peer may still store into its shared memory
+}
+
+// ------------------------------------------------------------------------------------------
+// The one-cluster solve with the vectors in DISTRIBUTED SHARED MEMORY.
+//
+// Up to 2048 sites per parity the solve is one cluster of <= 16 CTAs x 128 threads, one site per thread, the same in every
+// phase and iteration.  Every vector a neighbour reads -- r, the two direction buffers, t -- then fits the CTAs' shared memory
+// (4 vectors x 3 colours x 128 sites: 24 KB in fp64), each CTA holding the elements of its own sites: a neighbour element is
+// read from the owner's shared memory (mapa + ld.shared::cluster: ~215 cycles across CTAs, 38 inside the CTA, against a
+// 600-700-cycle L2 round trip for ld.global.cg), x and Ap never leave registers, and the site geometry (the sixteen neighbour
+// indices of the site as an odd and as an even site, their owners, the phases) is computed once, outside the iteration loop.
+// Most neighbours are in the CTA itself (x0, x1 and half of the x2 neighbours of 128 consecutive sites at 8^4; all of them at
+// 4^4, which is one CTA).  Links stay in global memory, L1-allocating: a CTA reads the same links in every iteration.
+// Same arithmetic in the same order as cg_persistent_body (and, per site, as dslash_kernel): same iterates.
+// ------------------------------------------------------------------------------------------
+template <typename T>
+struct ClusterHop {              // one neighbour of this thread's site: owner CTA and element inside the owner's arrays
+    unsigned short rank[8], off[8];        // hop = 2 mu + (0: forward, 1: backward)
+    unsigned neg;                          // bit hop: the hop's term enters with a minus sign (phase x seam)
+    int nb_global[4];                      // backward neighbour index (the backward link is stored there)
+    int x3;
+};
+
+template <typename T>
+__device__ __forceinline__ ClusterHop<T> cluster_hops(const Lattice &L, int parity, int cb, int spb)
+{
+    const SiteGeom g = site_geometry(L, parity, cb);
+    ClusterHop<T> h;
+    h.neg = 0u;
+#pragma unroll
+    for (int mu = 0; mu < 4; ++mu) {
+        h.rank[2 * mu] = (unsigned short)(g.nf[mu] / spb);     h.off[2 * mu] = (unsigned short)(g.nf[mu] % spb);
+        h.rank[2 * mu + 1] = (unsigned short)(g.nb[mu] / spb); h.off[2 * mu + 1] = (unsigned short)(g.nb[mu] % spb);
+        h.neg |= (g.sf[mu] < 0.f ? 1u : 0u) << (2 * mu);
+        h.neg |= (g.sb[mu] < 0.f ? 1u : 0u) << (2 * mu + 1);
+        h.nb_global[mu] = g.nb[mu];
+    }
+    h.x3 = g.x3;
+    return h;
+}
+
+// acc = (D in)(cb) with `in` in distributed shared memory ([3][BLOCK] per CTA); FUSE: the input is r + beta * in
+template <typename T, int NROW, int TG, bool FUSE, bool KEEP_L1, int BLOCK>
+__device__ __forceinline__ void cluster_site(typename Cplx<T>::type acc[3], const Lattice &L, int parity, int cb, const ClusterHop<T> &h,
+                                             const typename Cplx<T>::type *U, const typename Cplx<T>::type (*in)[BLOCK],
+                                             const typename Cplx<T>::type (*r)[BLOCK], T beta)
+{
+    typedef typename Cplx<T>::type C;
+    const size_t Vh = (size_t)L.Vh;
+    const uint64_t pol = l2_policy_evict_last();
+    const C *Uf = U + (size_t)(parity * 12 * NROW) * Vh + cb;
+    const C *Ub = U + (size_t)((1 - parity) * 12 * NROW) * Vh;
+    acc[0].x = acc[0].y = acc[1].x = acc[1].y = acc[2].x = acc[2].y = (T)0;
+#pragma unroll
+    for (int mu = 0; mu < 4; ++mu) {
+        const bool unit_f = TG && mu == 3 && h.x3 != 0;
+        const bool unit_b = TG && mu == 3 && h.x3 != 1;
+        C uf[9], ub[9], pf[3], pb[3];
+        if (!unit_f) {
+#pragma unroll
+            for (int k = 0; k < 3 * NROW; ++k) uf[k] = KEEP_L1 ? ld_keep(Uf + (size_t)(mu * 3 * NROW + k) * Vh, pol) : ld_stream(Uf + (size_t)(mu * 3 * NROW + k) * Vh, pol);
+        }
+        if (!unit_b) {
+#pragma unroll
+            for (int k = 0; k < 3 * NROW; ++k) ub[k] = KEEP_L1 ? ld_keep(Ub + (size_t)(mu * 3 * NROW + k) * Vh + h.nb_global[mu], pol) : ld_stream(Ub + (size_t)(mu * 3 * NROW + k) * Vh + h.nb_global[mu], pol);
+        }
+        const unsigned rf = h.rank[2 * mu], of = h.off[2 * mu], rb = h.rank[2 * mu + 1], ob = h.off[2 * mu + 1];
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            pf[c] = ld_shared_cluster(&in[c][of], rf);
+            pb[c] = ld_shared_cluster(&in[c][ob], rb);
+            if (FUSE) {
+                const C vf = ld_shared_cluster(&r[c][of], rf), vb = ld_shared_cluster(&r[c][ob], rb);
+                pf[c].x = fma(beta, pf[c].x, vf.x); pf[c].y = fma(beta, pf[c].y, vf.y);
+                pb[c].x = fma(beta, pb[c].x, vb.x); pb[c].y = fma(beta, pb[c].y, vb.y);
+            }
+        }
+        const unsigned nf = (h.neg >> (2 * mu)) & 1u, nb = (h.neg >> (2 * mu + 1)) & 1u;
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            pf[c].x = flip_sign(pf[c].x, nf); pf[c].y = flip_sign(pf[c].y, nf);
+            pb[c].x = flip_sign(pb[c].x, nb); pb[c].y = flip_sign(pb[c].y, nb);
+        }
+        if (!unit_f) { if (NROW == 2) reconstruct_third_row<C>(uf); mat_vec_acc<T, C>(acc, uf, pf); } else vec_acc<C>(acc, pf);
+        if (!unit_b) { if (NROW == 2) reconstruct_third_row<C>(ub); matdag_vec_acc<T, C>(acc, ub, pb); } else vec_acc<C>(acc, pb);
+    }
+}
+
+template <typename T, int NROW, int TG, int BLOCK>
+__device__ __forceinline__ void cg_cluster_body(const PersistArgs<T> &a)
+{
+    typedef typename Cplx<T>::type C;
+    // the links of a CTA's sites for BOTH phases (2 x 1152 B per site in fp64) stay in its L1 only if they fit: at 128 sites per CTA
+    // they do in fp32 (147 KB) and not in fp64 (295 KB), where the second phase streams its links past the L1 instead of evicting the first's
+    constexpr bool KEEP2 = sizeof(T) == 4;
+    __shared__ double smem[BLOCK / 32 + 1];
+    __shared__ double cl_slots[2 * CLUSTER_MAX_CTAS];
+    __shared__ __align__(16) C s_r[3][BLOCK], s_p[2][3][BLOCK], s_t[3][BLOCK];
+    const int Vh = a.L.Vh;
+    const size_t sVh = (size_t)Vh;
+    int spb = (Vh + (int)gridDim.x - 1) / (int)gridDim.x;      // sites per CTA, as in cg_persistent_body; <= BLOCK (host: ncta x BLOCK >= Vh)
+    spb += spb & 1;
+    const int site0 = (int)blockIdx.x * spb;
+    const int my_sites = Vh - site0 < spb ? (Vh - site0 > 0 ? Vh - site0 : 0) : spb;
+    const int tid = (int)threadIdx.x, cb = site0 + tid;
+    const bool active = tid < my_sites;
+    const int gtid = blockIdx.x * BLOCK + threadIdx.x;
+    unsigned epoch = 0;
+
+    // the thread's site: its vectors into shared memory / registers, its geometry as an odd (phase 1) and as an even site (phase 2)
+    C vx[3];
+    ClusterHop<T> h_odd, h_even;
+    if (active) {
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            s_r[c][tid] = a.r[(size_t)c * sVh + cb];
+            s_p[0][c][tid] = a.p[(size_t)c * sVh + cb];
+            vx[c] = a.x[(size_t)c * sVh + cb];
+        }
+        h_odd = cluster_hops<T>(a.L, 1, cb, spb);
+        h_even = cluster_hops<T>(a.L, 0, cb, spb);
+    }
+    cluster_barrier();          // every CTA runs and has filled its arrays before anyone reads them or stores into its slots
+
+    double rr = a.scal->rr;
+    const double tol2bb = a.scal->tol2bb;
+    const int maxiter = a.scal->maxiter;
+    int k = a.scal->k, flag = a.scal->flag;
+    double alpha = 0.0, beta = 0.0, pAp = 0.0;
+
+    unsigned long long *tl = nullptr;
+    if (a.timeline && threadIdx.x == 0 && (blockIdx.x == 0 || blockIdx.x == gridDim.x - 1))
+        tl = a.timeline + (blockIdx.x == 0 ? 0 : TIMELINE_ITERS * TIMELINE_STAMPS);
+    int it = 0;
+#define QCD_STAMP(i) do { if (tl && it < TIMELINE_ITERS) tl[it * TIMELINE_STAMPS + (i)] = global_ns(); } while (0)
+
+    int old = 0;                                               // s_p[old] is p of the previous iteration, s_p[old ^ 1] receives the new one
+    while (flag == 0) {
+        QCD_STAMP(0);
+        // phase 1: p' = r + beta p (own site, into the other buffer), t = D_oe p' with p' formed on the fly at the neighbours
+        const T be = (T)beta;
+        const int cur = old ^ 1;
+        C vp[3];                                               // p' of the own site: phases 2 and 3 use it from registers
+        if (active) {
+            C acc[3];
+            cluster_site<T, NROW, TG, true, true, BLOCK>(acc, a.L, 1, cb, h_odd, a.U, s_p[old], s_r, be);
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+                const C po = s_p[old][c][tid], ro = s_r[c][tid];
+                vp[c].x = fma(be, po.x, ro.x); vp[c].y = fma(be, po.y, ro.y);
+                s_p[cur][c][tid] = vp[c];
+                s_t[c][tid] = acc[c];
+            }
+        }
+        QCD_STAMP(1);
+        cluster_barrier();                                     // t and p' are complete everywhere
+        QCD_STAMP(2);
+        // phase 2: Ap = m^2 p' - D_eo t (registers), partial Re<p',Ap>
+        double dot = 0.0;
+        C va[3];
+        if (active) {
+            C acc[3];
+            cluster_site<T, NROW, TG, false, KEEP2, BLOCK>(acc, a.L, 0, cb, h_even, a.U, s_t, s_t, (T)0);
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+                va[c].x = fma(a.m2, vp[c].x, -acc[c].x);
+                va[c].y = fma(a.m2, vp[c].y, -acc[c].y);
+                dot += (double)vp[c].x * (double)va[c].x + (double)vp[c].y * (double)va[c].y;
+            }
+        }
+        const double dot_block = block_sum<BLOCK>(dot, smem);
+        QCD_STAMP(3);
+        pAp = solve_barrier<BLOCK, true>(dot_block, ++epoch, a.partials, smem, cl_slots);
+        QCD_STAMP(4);
+        if (!(pAp > 0.0)) { flag = 3; break; }                     // breakdown: uniform across the cluster
+        alpha = rr / pAp;
+        QCD_STAMP(5);
+        // phase 3: x += alpha p' (registers), r -= alpha Ap (own shared memory), partial <r,r>
+        const T al = (T)alpha;
+        double nrm = 0.0;
+        if (active) {
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+                C vr = s_r[c][tid];
+                vx[c].x = fma(al, vp[c].x, vx[c].x); vx[c].y = fma(al, vp[c].y, vx[c].y);
+                vr.x = fma(-al, va[c].x, vr.x); vr.y = fma(-al, va[c].y, vr.y);
+                s_r[c][tid] = vr;
+                nrm += (double)vr.x * (double)vr.x + (double)vr.y * (double)vr.y;
+            }
+        }
+        __syncthreads();                                           // smem of the previous barrier has been read by everyone
+        const double nrm_block = block_sum<BLOCK>(nrm, smem);
+        QCD_STAMP(6);
+        const double rr_new = solve_barrier<BLOCK, true>(nrm_block, ++epoch, a.partials, smem, cl_slots);
+        QCD_STAMP(7);
+        beta = rr_new / rr;
+        rr = rr_new;
+        k += 1;
+        if (gtid == 0) {                                           // residual history (qcd_cg_history)
+            double *const hist = a.scal->hist;
+            if (hist && k <= a.scal->hist_cap) hist[k - 1] = rr_new;
+        }
+        QCD_STAMP(8);
+        ++it;
+        if (rr_new != rr_new) flag = 3;
+        else if (rr_new <= tol2bb) flag = 1;
+        else if (k >= maxiter) flag = 2;
+        if (flag != 0) break;
+        old = cur;
+    }
+#undef QCD_STAMP
+    if (active) {
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            a.x[(size_t)c * sVh + cb] = vx[c];
+            a.r[(size_t)c * sVh + cb] = s_r[c][tid];               // the workspace keeps the last residual, as the other loops leave it
+        }
+    }
+    if (gtid == 0) {
+        CgScalars *s = a.scal;
+        s->rr = rr; s->pAp = pAp; s->alpha = alpha; s->beta = beta; s->k = k; s->flag = flag;
+    }
+    cluster_barrier();                              // no CTA exits while a peer may still read or store into its shared memory
 }
 
 // cooperative launch, any number of co-resident blocks
 template <typename T, int NROW, int TG>
 __global__ void __launch_bounds__(PersistBlock<T>::value, PersistMinB<T>::value) cg_persistent_kernel(const PersistArgs<T> a)
 {
-    cg_persistent_body<T, NROW, TG, PersistBlock<T>::value, false>(a);
+    cg_persistent_body<T, NROW, TG, PersistBlock<T>::value>(a);
 }
 
 // ONE cluster of 1 .. 16 CTAs (cluster dimension = grid dimension, set at launch)
 template <typename T, int NROW, int TG>
 __global__ void __launch_bounds__(ClusterBlock<T>::value, 1) cg_cluster_kernel(const PersistArgs<T> a)
 {
-    cg_persistent_body<T, NROW, TG, ClusterBlock<T>::value, true>(a);
+    cg_cluster_body<T, NROW, TG, ClusterBlock<T>::value>(a);
 }
 
 } // namespace qcd
