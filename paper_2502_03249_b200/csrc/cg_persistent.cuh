@@ -70,23 +70,26 @@ __device__ __forceinline__ void st_shared_cluster(double *local, unsigned rank, 
     asm volatile("st.shared::cluster.f64 [%0], %1;" :: "r"(ra), "d"(v) : "memory");
 }
 
-// load a complex number from the shared memory of CTA `rank` of the cluster, at the address that `local` has in this CTA
-__device__ __forceinline__ double2 ld_shared_cluster(const double2 *local, unsigned rank)
+// the address, in the cluster's shared window, that the shared-memory address `local` of this CTA has in CTA `rank`
+__device__ __forceinline__ unsigned cluster_map(unsigned local, unsigned rank)
 {
-    const unsigned la = (unsigned)__cvta_generic_to_shared(local);
     unsigned ra;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(ra) : "r"(local), "r"(rank));
+    return ra;
+}
+// a complex number at cluster-window address `addr` + OFF bytes (OFF a compile-time constant: an immediate of the load)
+template <int OFF>
+__device__ __forceinline__ double2 ld_cluster_at(unsigned addr, double2)
+{
     double2 v;
-    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(ra) : "r"(la), "r"(rank));
-    asm volatile("ld.shared::cluster.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "r"(ra) : "memory");
+    asm volatile("ld.shared::cluster.v2.f64 {%0, %1}, [%2 + %3];" : "=d"(v.x), "=d"(v.y) : "r"(addr), "n"(OFF) : "memory");
     return v;
 }
-__device__ __forceinline__ float2 ld_shared_cluster(const float2 *local, unsigned rank)
+template <int OFF>
+__device__ __forceinline__ float2 ld_cluster_at(unsigned addr, float2)
 {
-    const unsigned la = (unsigned)__cvta_generic_to_shared(local);
-    unsigned ra;
     float2 v;
-    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(ra) : "r"(la), "r"(rank));
-    asm volatile("ld.shared::cluster.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "r"(ra) : "memory");
+    asm volatile("ld.shared::cluster.v2.f32 {%0, %1}, [%2 + %3];" : "=f"(v.x), "=f"(v.y) : "r"(addr), "n"(OFF) : "memory");
     return v;
 }
 
@@ -390,7 +393,7 @@ __device__ __forceinline__ void cg_persistent_body(const PersistArgs<T> &a)
 // Up to 2048 sites per parity the solve is one cluster of <= 16 CTAs x 128 threads, one site per thread, the same in every
 // phase and iteration.  Every vector a neighbour reads -- r, the two direction buffers, t -- then fits the CTAs' shared memory
 // (4 vectors x 3 colours x 128 sites: 24 KB in fp64), each CTA holding the elements of its own sites: a neighbour element is
-// read from the owner's shared memory (mapa + ld.shared::cluster: ~215 cycles across CTAs, 38 inside the CTA, against a
+// read from the owner's shared memory (one mapa per hop + ld.shared::cluster with the colour as an immediate: ~215 cycles across CTAs, 38 inside the CTA, against a
 // 600-700-cycle L2 round trip for ld.global.cg), x and Ap never leave registers, and the site geometry (the sixteen neighbour
 // indices of the site as an odd and as an even site, their owners, the phases) is computed once, outside the iteration loop.
 // Most neighbours are in the CTA itself (x0, x1 and half of the x2 neighbours of 128 consecutive sites at 8^4; all of them at
@@ -426,9 +429,10 @@ __device__ __forceinline__ ClusterHop<T> cluster_hops(const Lattice &L, int pari
 // acc = (D in)(cb) with `in` in distributed shared memory ([3][BLOCK] per CTA); FUSE: the input is r + beta * in
 template <typename T, int NROW, int TG, bool FUSE, bool KEEP_L1, int BLOCK>
 __device__ __forceinline__ void cluster_site(typename Cplx<T>::type acc[3], const Lattice &L, int parity, int cb, const ClusterHop<T> &h,
-                                             const typename Cplx<T>::type *U, const typename Cplx<T>::type (*in)[BLOCK],
-                                             const typename Cplx<T>::type (*r)[BLOCK], T beta)
+                                             const typename Cplx<T>::type *U, unsigned in_saddr, unsigned r_saddr, T beta)
 {
+    // in_saddr / r_saddr: shared-window addresses, in THIS CTA, of element [0][0] of the [3][BLOCK] arrays `in` and `r`; the same arrays of
+    // the owner CTA are reached with ONE mapa per hop, the three colours are immediates of the loads
     typedef typename Cplx<T>::type C;
     const size_t Vh = (size_t)L.Vh;
     const uint64_t pol = l2_policy_evict_last();
@@ -449,14 +453,19 @@ __device__ __forceinline__ void cluster_site(typename Cplx<T>::type acc[3], cons
             for (int k = 0; k < 3 * NROW; ++k) ub[k] = KEEP_L1 ? ld_keep(Ub + (size_t)(mu * 3 * NROW + k) * Vh + h.nb_global[mu], pol) : ld_stream(Ub + (size_t)(mu * 3 * NROW + k) * Vh + h.nb_global[mu], pol);
         }
         const unsigned rf = h.rank[2 * mu], of = h.off[2 * mu], rb = h.rank[2 * mu + 1], ob = h.off[2 * mu + 1];
+        constexpr int COL = BLOCK * (int)sizeof(C);             // bytes between colours
+        const unsigned af = cluster_map(in_saddr, rf) + of * (unsigned)sizeof(C), ab = cluster_map(in_saddr, rb) + ob * (unsigned)sizeof(C);
+        pf[0] = ld_cluster_at<0>(af, C()); pf[1] = ld_cluster_at<COL>(af, C()); pf[2] = ld_cluster_at<2 * COL>(af, C());
+        pb[0] = ld_cluster_at<0>(ab, C()); pb[1] = ld_cluster_at<COL>(ab, C()); pb[2] = ld_cluster_at<2 * COL>(ab, C());
+        if (FUSE) {
+            const unsigned d = r_saddr - in_saddr;              // the same displacement in every CTA
+            C vf[3], vb[3];
+            vf[0] = ld_cluster_at<0>(af + d, C()); vf[1] = ld_cluster_at<COL>(af + d, C()); vf[2] = ld_cluster_at<2 * COL>(af + d, C());
+            vb[0] = ld_cluster_at<0>(ab + d, C()); vb[1] = ld_cluster_at<COL>(ab + d, C()); vb[2] = ld_cluster_at<2 * COL>(ab + d, C());
 #pragma unroll
-        for (int c = 0; c < 3; ++c) {
-            pf[c] = ld_shared_cluster(&in[c][of], rf);
-            pb[c] = ld_shared_cluster(&in[c][ob], rb);
-            if (FUSE) {
-                const C vf = ld_shared_cluster(&r[c][of], rf), vb = ld_shared_cluster(&r[c][ob], rb);
-                pf[c].x = fma(beta, pf[c].x, vf.x); pf[c].y = fma(beta, pf[c].y, vf.y);
-                pb[c].x = fma(beta, pb[c].x, vb.x); pb[c].y = fma(beta, pb[c].y, vb.y);
+            for (int c = 0; c < 3; ++c) {
+                pf[c].x = fma(beta, pf[c].x, vf[c].x); pf[c].y = fma(beta, pf[c].y, vf[c].y);
+                pb[c].x = fma(beta, pb[c].x, vb[c].x); pb[c].y = fma(beta, pb[c].y, vb[c].y);
             }
         }
         const unsigned nf = (h.neg >> (2 * mu)) & 1u, nb = (h.neg >> (2 * mu + 1)) & 1u;
@@ -518,6 +527,8 @@ __device__ __forceinline__ void cg_cluster_body(const PersistArgs<T> &a)
     int it = 0;
 #define QCD_STAMP(i) do { if (tl && it < TIMELINE_ITERS) tl[it * TIMELINE_STAMPS + (i)] = global_ns(); } while (0)
 
+    const unsigned sa_r = (unsigned)__cvta_generic_to_shared(&s_r[0][0]), sa_p = (unsigned)__cvta_generic_to_shared(&s_p[0][0][0]),
+                   sa_t = (unsigned)__cvta_generic_to_shared(&s_t[0][0]);
     int old = 0;                                               // s_p[old] is p of the previous iteration, s_p[old ^ 1] receives the new one
     while (flag == 0) {
         QCD_STAMP(0);
@@ -527,7 +538,7 @@ __device__ __forceinline__ void cg_cluster_body(const PersistArgs<T> &a)
         C vp[3];                                               // p' of the own site: phases 2 and 3 use it from registers
         if (active) {
             C acc[3];
-            cluster_site<T, NROW, TG, true, true, BLOCK>(acc, a.L, 1, cb, h_odd, a.U, s_p[old], s_r, be);
+            cluster_site<T, NROW, TG, true, true, BLOCK>(acc, a.L, 1, cb, h_odd, a.U, sa_p + (unsigned)old * (unsigned)sizeof(s_p[0]), sa_r, be);
 #pragma unroll
             for (int c = 0; c < 3; ++c) {
                 const C po = s_p[old][c][tid], ro = s_r[c][tid];
@@ -544,7 +555,7 @@ __device__ __forceinline__ void cg_cluster_body(const PersistArgs<T> &a)
         C va[3];
         if (active) {
             C acc[3];
-            cluster_site<T, NROW, TG, false, KEEP2, BLOCK>(acc, a.L, 0, cb, h_even, a.U, s_t, s_t, (T)0);
+            cluster_site<T, NROW, TG, false, KEEP2, BLOCK>(acc, a.L, 0, cb, h_even, a.U, sa_t, sa_t, (T)0);
 #pragma unroll
             for (int c = 0; c < 3; ++c) {
                 va[c].x = fma(a.m2, vp[c].x, -acc[c].x);
