@@ -1019,7 +1019,10 @@ static qcd_status cg_persistent_launch(qcd_ctx *c, bool probe_only, bool *ok)
     if (c->L.Vh <= CLUSTER_MAX_SITES && c->loop_cluster_ok) {
         auto kernel = cg_cluster_kernel<T, NROW, TG>;
         int ncta = 1;
-        while (ncta * CLUSTER_BLOCK < wanted_threads && ncta < CLUSTER_MAX_CTAS) ncta *= 2;
+        // sites per CTA: as many as the block has threads, but in fp64 at most 64 while CTAs are to be had -- the links of 64 sites for both
+        // phases (147 KB) fit the L1 next to the vectors' shared memory, those of 128 (295 KB) do not and come from the L2 every iteration
+        const int per_cta = sizeof(T) == 8 ? CLUSTER_BLOCK / 2 : CLUSTER_BLOCK;
+        while (ncta * per_cta < wanted_threads && ncta < CLUSTER_MAX_CTAS) ncta *= 2;
         cudaLaunchConfig_t cfg;
         memset(&cfg, 0, sizeof cfg);
         cfg.gridDim = dim3(ncta); cfg.blockDim = dim3(CLUSTER_BLOCK); cfg.dynamicSmemBytes = 0; cfg.stream = c->stream;
