@@ -194,11 +194,10 @@ __device__ __forceinline__ void persistent_site(typename Cplx<T>::type acc[3], c
     const C *Uf = U + (size_t)(parity * 12 * NROW) * Vh + cb;
     const C *Ub = U + (size_t)((1 - parity) * 12 * NROW) * Vh;
     acc[0].x = acc[0].y = acc[1].x = acc[1].y = acc[2].x = acc[2].y = (T)0;
-#pragma unroll
-    for (int mu = 0; mu < 4; ++mu) {
+    // links requested one direction ahead, two sets of link registers used in turn (see cluster_site)
+    auto load_links = [&](int mu, C (&uf)[9], C (&ub)[9]) {
         const bool unit_f = TG && mu == 3 && g.x3 != 0;
         const bool unit_b = TG && mu == 3 && g.x3 != 1;
-        C uf[9], ub[9], pf[3], pb[3];
         if (!unit_f) {
 #pragma unroll
             for (int k = 0; k < 3 * NROW; ++k) uf[k] = KEEP_L1 ? ld_keep(Uf + (size_t)(mu * 3 * NROW + k) * Vh, pol) : ld_stream(Uf + (size_t)(mu * 3 * NROW + k) * Vh, pol);
@@ -207,6 +206,11 @@ __device__ __forceinline__ void persistent_site(typename Cplx<T>::type acc[3], c
 #pragma unroll
             for (int k = 0; k < 3 * NROW; ++k) ub[k] = KEEP_L1 ? ld_keep(Ub + (size_t)(mu * 3 * NROW + k) * Vh + g.nb[mu], pol) : ld_stream(Ub + (size_t)(mu * 3 * NROW + k) * Vh + g.nb[mu], pol);
         }
+    };
+    auto hops = [&](int mu, C (&uf)[9], C (&ub)[9]) {
+        const bool unit_f = TG && mu == 3 && g.x3 != 0;
+        const bool unit_b = TG && mu == 3 && g.x3 != 1;
+        C pf[3], pb[3];
         const unsigned nf = g.sf[mu] < 0.f ? 1u : 0u, nb = g.sb[mu] < 0.f ? 1u : 0u;
 #pragma unroll
         for (int c = 0; c < 3; ++c) {
@@ -225,7 +229,16 @@ __device__ __forceinline__ void persistent_site(typename Cplx<T>::type acc[3], c
         }
         if (!unit_f) { if (NROW == 2) reconstruct_third_row<C>(uf); mat_vec_acc<T, C>(acc, uf, pf); } else vec_acc<C>(acc, pf);
         if (!unit_b) { if (NROW == 2) reconstruct_third_row<C>(ub); matdag_vec_acc<T, C>(acc, ub, pb); } else vec_acc<C>(acc, pb);
-    }
+    };
+    C ufA[9], ubA[9], ufB[9], ubB[9];
+    load_links(0, ufA, ubA);
+    load_links(1, ufB, ubB);
+    hops(0, ufA, ubA);
+    load_links(2, ufA, ubA);
+    hops(1, ufB, ubB);
+    load_links(3, ufB, ubB);
+    hops(2, ufA, ubA);
+    hops(3, ufB, ubB);
 }
 
 // The grid version (cooperative launch): vectors in global memory, read through the L2.
